@@ -154,6 +154,24 @@ void oracle_set_state(oracle_sim* h, const double* x0, const double* v0, const d
   h->H_done = 0;
 }
 
+// Test hook: replace the A0 products (initial frames d1 [B][3][N], grasp-local coordinates q [B][G][M][3]) after
+// oracle_set_state, so that finite differences in x0 can hold them fixed exactly as the reverse pass does
+// ("no gradient through A0", Backward).  Either may be NULL.
+void oracle_override_init(oracle_sim* h, const double* d1, const double* q) {
+  const Config& c = h->c; const int N = c.N, E = c.E(), GM = c.G * c.n_grasp_max;
+  for (int b = 0; b < h->B; ++b) {
+    EnvD& e = h->env[b];
+    if (d1) for (int j = 0; j < E; ++j) e.s0.d1[j] = mkv(d1[(size_t)b * 3 * N + j], d1[(size_t)b * 3 * N + N + j], d1[(size_t)b * 3 * N + 2 * N + j]);
+    if (q) for (int k = 0; k < GM; ++k) e.sc.q[k] = mkv(q[((size_t)b * GM + k) * 3], q[((size_t)b * GM + k) * 3 + 1], q[((size_t)b * GM + k) * 3 + 2]);
+    e.cur = e.s0;
+  }
+}
+void oracle_get_grasp_local(oracle_sim* h, double* q /* [B][G][M][3] */) {
+  const int GM = h->c.G * h->c.n_grasp_max;
+  for (int b = 0; b < h->B; ++b)
+    for (int k = 0; k < GM; ++k) { const Vec3<double>& v = h->env[b].sc.q[k]; double* o = q + ((size_t)b * GM + k) * 3; o[0] = v.x; o[1] = v.y; o[2] = v.z; }
+}
+
 void oracle_set_actions(oracle_sim* h, const double* actions /* [H][B][G][6] */, int32_t horizon) {
   h->actions.assign(actions, actions + (size_t)horizon * h->B * h->c.G * 6);
   h->H_actions = horizon;

@@ -62,7 +62,7 @@ def make_config(cfg: dict) -> OracleConfig:
 class OracleSim:
     """fp64 CPU rollout + tape-AD backward for a problem dict (see workloads/configs.py). `envs` selects a subset."""
 
-    def __init__(self, problem: dict, envs=None):
+    def __init__(self, problem: dict, envs=None, frozen_init=None):
         L = lib()
         cfg = dict(problem["config"])
         B_all = cfg["batch"]
@@ -87,10 +87,20 @@ class OracleSim:
         kb = problem.get("kappa_bar0")
         kb = None if kb is None else _d(kb[self.envs])
         L.oracle_set_state(self.h, _ptr(_d(problem["x0"][self.envs])), _ptr(_d(problem["v0"][self.envs])), _ptr(kb))
+        if frozen_init is not None:      # test hook: hold the A0 products (frames, grasp-local coordinates) fixed
+            d1, q = frozen_init.get("d1"), frozen_init.get("q")
+            L.oracle_override_init(self.h, _ptr(None if d1 is None else _d(d1)), _ptr(None if q is None or self.G == 0 else _d(q)))
         self.H = int(problem.get("horizon", 0))
         self.stride = int(problem.get("checkpoint_stride", 0))
         if self.G > 0 and problem.get("actions") is not None:
             self.set_actions(problem["actions"][:, self.envs])
+
+    def init_products(self):
+        """A0 products: initial frames d1 [B][3][N] (call before rollout) and grasp-local coordinates q [B][G][M][3]."""
+        q = np.zeros((self.B, max(self.G, 0), self.M, 3))
+        if self.G > 0:
+            lib().oracle_get_grasp_local(self.h, _ptr(q))
+        return {"d1": self.state()["d1"], "q": q}
 
     def set_actions(self, actions):
         a = _d(actions)
