@@ -1,0 +1,141 @@
+/* dlo.h — C-ABI of the B200-native batched differentiable rod step (DLO-Lab hot path).
+ *
+ * What the library computes.  One "env" is one discretised deformable linear object (rope / band): N vertices
+ * x_i with adapted frames per edge (Eq.1), advanced by symplectic Euler (L97) in frames of
+ * `dt` made of `n_substeps` substeps (L438).  Each substep is, in this order (paper silent on the order;
+ * DESIGN.md reading R-31): gripper kinematics (L129) -> internal forces: gravity, stretching Eq.2-3 (L344-351,
+ * stretch mode ENERGY) and bending Eq.4-7 (L353-372) -> damped velocity update -> predict -> N_C iterations of
+ * {inextensibility projection Eq.10 (L383-392) with optional compliance, red/black edge order; segment-segment
+ * self-contact projection Eq.13 (L406-408)} -> velocity reconciliation + self-contact Coulomb friction (L410)
+ * -> soft coupling against rigid primitives and gripper fingers (L103) -> commit -> frame transport and
+ * bending plasticity Eq.11 (L394-398).  Ring topology initialises frames with the holonomy correction Eq.12
+ * (L400-404).  `dlo_backward` is the exact reverse-mode derivative of that discrete map (branches frozen at
+ * their forward outcome) under gradient checkpointing: one state per `checkpoint_stride` steps kept, segments
+ * replayed in reverse (L115).
+ *
+ * Conventions
+ *   - All arithmetic on the GPU is fp32.  B = batch, N = n_verts, E = N-1 (open) or N (ring), G = n_grippers,
+ *     M = n_grasp_max, K = n_primitives, H = horizon (steps = frames).
+ *   - Every array argument says "dev" (CUDA device pointer, 16-byte aligned) or "host".  Layouts are dense,
+ *     row-major, last index fastest: x, v, d1 are [B][3][N] (SoA per env; d1 uses the first E columns);
+ *     kappa_bar is [B][2][N]; actions are [H][B][G][6] = (position p, rotation vector rho) of each gripper
+ *     reached exactly at the END of step t (R-20).
+ *   - Ownership: the caller owns every buffer it passes.  The library reads / writes them asynchronously on
+ *     the stream given at create and keeps no pointer after the call returns, except `actions` (borrowed until
+ *     the next dlo_set_actions / dlo_destroy: dlo_backward replays them).  Checkpoints, tape and per-env
+ *     constants live in library-owned device memory (size: dlo_scratch_bytes).
+ *   - Errors: every call returns a dlo_status; nothing aborts or throws across the ABI; a failed call leaves
+ *     the handle usable.  dlo_last_error() returns a thread-local message for the last failing call.
+ *   - Threading: one handle <-> one stream; calls are stream-ordered and (except the *_host calls and
+ *     dlo_check_numerics) do not synchronise the host.
+ *   - There is no CPU fallback: without a CUDA device dlo_create returns DLO_ERR_CUDA.
+ */
+#ifndef DLO_H_
+#define DLO_H_
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dlo_sim dlo_sim;   /* opaque, library-owned */
+typedef int32_t dlo_status;
+
+enum { DLO_OK = 0, DLO_ERR_INVALID_ARG = -1, DLO_ERR_BAD_STATE = -2 /* call order */, DLO_ERR_CUDA = -3,
+       DLO_ERR_OOM = -4, DLO_ERR_UNSUPPORTED = -5, DLO_ERR_NUMERIC = -6 /* non-finite state / candidate overflow */ };
+enum { DLO_OPEN = 0, DLO_RING = 1 };
+enum { DLO_STRETCH_ENERGY = 0 /* Eq.2-3 force */, DLO_STRETCH_PROJECT = 1 /* Eq.10 projection (+compliance) */ };
+enum { DLO_PRIM_PLANE = 0, DLO_PRIM_CAPSULE = 1, DLO_PRIM_CYLINDER = 2, DLO_PRIM_BOX = 3 };
+
+#define DLO_MAX_VERTS 256       /* one warp per env, <= 8 vertices per lane */
+#define DLO_MAX_GRIPPERS 4
+#define DLO_MAX_PRIMITIVES 16
+#define DLO_PRIM_NPARAM 10
+#define DLO_N_MATERIAL_GRADS 5  /* stretch, bend, damping, yield, creep */
+
+/* Host POD, copied at create.  Limits: 3 <= n_verts <= DLO_MAX_VERTS (ring: >= 4), n_grippers <= 4,
+ * n_primitives <= 16, n_substeps >= 1, n_proj_iters >= 0. */
+typedef struct {
+  int32_t batch, n_verts, topology, n_substeps /* 5, L438 */, n_proj_iters /* N_C, L392 */, stretch_mode;
+  int32_t enable_plasticity /* Eq.11 */, enable_self_contact /* Eq.13 */, self_skip /* min cyclic edge-index distance, 2 */;
+  int32_t n_grippers, n_grasp_max, n_primitives;
+  int32_t kappa_bar_from_x0;   /* 1: dlo_set_state(kappa_bar0 = NULL) takes the rest curvature of x0 instead of 0 */
+  float dt, gravity[3], rope_radius, contact_softness /* eps_s of L103 */, influence_threshold /* 0.1, L103 */,
+      restitution;
+} dlo_config;
+
+/* DEVICE pointers, each [B] fp32, copied at create.  `stretch` is k_s (mode ENERGY, Eq.3) or the compliance c in
+ * m/N (mode PROJECT; 0 = Eq.10 verbatim).  bend_stiffness is alpha = E A r^2 / 4 of Eq.7.  yield_curv in rad/m
+ * (compared as sigma_y * l_bar with the integrated curvature of Eq.5), creep_rate = r_c of Eq.11. */
+typedef struct {
+  const float *mass_per_vertex, *rest_edge_len, *stretch, *bend_stiffness, *damping, *yield_curv, *creep_rate,
+      *mu_rigid, *mu_self;
+} dlo_material;
+
+/* Create a simulator for `batch` independent envs on `cuda_stream` (a cudaStream_t, NULL = default stream).
+ * Fails with DLO_ERR_INVALID_ARG on out-of-range sizes, DLO_ERR_CUDA without a device, DLO_ERR_OOM. */
+dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* cuda_stream, dlo_sim** out);
+dlo_status dlo_destroy(dlo_sim* sim);
+
+/* Scene.  Call before dlo_set_state (A0 captures grasp-local coordinates there).
+ * pins: dev [B][N] uint8, non-zero = vertex fixed in space (w = 0).
+ * primitives: types host [K] (same for all envs), params dev [B][K][10]:
+ *   PLANE n(3), o          CAPSULE a(3), b(3), R          CYLINDER centre(3), unit axis(3), R, half-height
+ *   BOX centre(3), half-extents(3), rotation vector(3).   All fixed in space (L103, kinematic bodies only).
+ * grippers: init_pose dev [B][G][6] = a_{-1}; finger_geom dev [B][G][4] = gap, length, radius, pad (two capsule
+ *   fingers from p + R(+-gap/2,0,0) to p + R(+-gap/2,0,length)); grasp_verts dev [B][G][M] int32, -1 = none:
+ *   vertices carried rigidly by the gripper (kinematic, L103). */
+dlo_status dlo_set_pins(dlo_sim* sim, const uint8_t* pinned);
+dlo_status dlo_set_primitives(dlo_sim* sim, const int32_t* types, const float* params);
+dlo_status dlo_set_grippers(dlo_sim* sim, const float* init_pose, const float* finger_geom, const int32_t* grasp_verts);
+
+/* A0: initial state x0, v0 dev [B][3][N]; kappa_bar0 dev [B][2][N] or NULL.  Builds the frames by parallel
+ * transport (ring: Eq.12) and the grasp-local coordinates. */
+dlo_status dlo_set_state(dlo_sim* sim, const float* x0, const float* v0, const float* kappa_bar0);
+
+/* actions dev [H][B][G][6]; borrowed (see Ownership).  Ignored when n_grippers == 0 (may be NULL). */
+dlo_status dlo_set_actions(dlo_sim* sim, const float* actions, int32_t horizon);
+
+/* Roll the state set by dlo_set_state forward by `horizon` steps.  checkpoint_stride > 0 keeps the state every
+ * `stride` steps for dlo_backward (L115); 0 = forward only.  DLO_ERR_INVALID_ARG if horizon exceeds the actions. */
+dlo_status dlo_rollout_forward(dlo_sim* sim, int32_t horizon, int32_t checkpoint_stride);
+
+/* Current state; each pointer dev, may be NULL.  x, v, d1: [B][3][N]; kappa_bar: [B][2][N]. */
+dlo_status dlo_get_state(dlo_sim* sim, float* x, float* v, float* d1, float* kappa_bar);
+
+/* Reverse pass of the last checkpointed rollout.  Seeds dL/dx_T, dL/dv_T dev [B][3][N] (NULL = 0).  Outputs
+ * (dev, each may be NULL, WRITTEN not accumulated): g_actions [H][B][G][6], g_x0, g_v0 [B][3][N],
+ * g_material [B][5] = d/d(stretch, bend_stiffness, damping, yield_curv, creep_rate).  The initial frames and
+ * rest curvature are independent inputs (no gradient through A0).  DLO_ERR_BAD_STATE without a checkpointed
+ * rollout. */
+dlo_status dlo_backward(dlo_sim* sim, const float* dL_dx_T, const float* dL_dv_T, float* g_actions, float* g_x0,
+                        float* g_v0, float* g_material);
+
+/* Host-buffer convenience calls (the end-to-end path): pageable or pinned HOST pointers, copies included, and
+ * the call returns after the results have landed.  dlo_rollout_forward_host = set_state + set_actions +
+ * rollout_forward + read-back of x_T, v_T (either may be NULL).  dlo_backward_host = seeds up, dlo_backward,
+ * gradients down (any may be NULL). */
+dlo_status dlo_rollout_forward_host(dlo_sim* sim, const float* x0, const float* v0, const float* kappa_bar0,
+                                    const float* actions, int32_t horizon, int32_t checkpoint_stride, float* x_T,
+                                    float* v_T);
+dlo_status dlo_backward_host(dlo_sim* sim, const float* dL_dx_T, const float* dL_dv_T, float* g_actions, float* g_x0,
+                             float* g_v0, float* g_material);
+
+/* Synchronises the stream; DLO_ERR_NUMERIC if any env saw a non-finite state or overflowed its self-contact
+ * candidate list since dlo_set_state; n_bad (host, may be NULL) receives the number of such envs. */
+dlo_status dlo_check_numerics(dlo_sim* sim, int32_t* n_bad);
+
+/* Device bytes the library allocates for this config / rollout shape (constants + checkpoints + tape). */
+size_t dlo_scratch_bytes(const dlo_config* cfg, int32_t horizon, int32_t checkpoint_stride);
+
+/* Number of kernel launches issued on this handle since create (bench.py's gpu_launches). */
+int64_t dlo_launch_count(const dlo_sim* sim);
+
+const char* dlo_last_error(void);
+const char* dlo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DLO_H_ */

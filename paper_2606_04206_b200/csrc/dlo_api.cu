@@ -1,0 +1,340 @@
+// dlo_api.cu — host driver behind the C-ABI of include/dlo.h: handle, device buffers, launch schedule of the
+// forward segment kernel and of the replay + adjoint kernels (gradient checkpointing).
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <string>
+#include <vector>
+
+#include "../../include/dlo.h"
+#include "rod_kernels.cuh"
+#include "rod_adjoint.cuh"
+
+using namespace dlo;
+
+static thread_local std::string g_err;
+static dlo_status fail(dlo_status code, const std::string& msg) { g_err = msg; return code; }
+#define CU(call)                                                                                        \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess) {                                                                            \
+      dlo_status c_ = (e_ == cudaErrorMemoryAllocation) ? DLO_ERR_OOM : DLO_ERR_CUDA;                    \
+      return fail(c_, std::string(#call) + ": " + cudaGetErrorString(e_));                              \
+    }                                                                                                   \
+  } while (0)
+
+struct dlo_sim {
+  dlo_config cfg;
+  cudaStream_t stream;
+  KParams P;                      // kernel parameter block (pointers filled as buffers appear)
+  int VPL, smem_fwd, smem_adj;
+  size_t blk;                     // floats per env state block
+  // library-owned device memory
+  float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
+  float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr;
+  uint8_t *kin = nullptr, *pins = nullptr;
+  int *grasp = nullptr, *flags = nullptr;
+  size_t ckpt_blocks = 0, tape_blocks = 0;
+  const float* actions = nullptr;   // borrowed
+  int H_actions = 0, H_done = 0, stride = 0;
+  bool have_state = false, have_prims = false, have_grippers = false;
+  int64_t launches = 0;
+  // staging for the *_host calls
+  float *hx0 = nullptr, *hv0 = nullptr, *hkb = nullptr, *hact = nullptr, *hseed_x = nullptr, *hseed_v = nullptr;
+  float *hg_act = nullptr, *hg_x0 = nullptr, *hg_v0 = nullptr, *hg_mat = nullptr, *hxT = nullptr, *hvT = nullptr;
+  int hact_H = 0;
+};
+
+static int vpl_for(int N) { return 2 * ((N + 63) / 64); }
+static int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+// per-warp shared-memory layout (float offsets); `adjoint` adds the reverse-pass scratch
+static int smem_layout(KParams& P, int VPL, bool adjoint) {
+  const int NP = 32 * VPL;
+  int o = 0;
+  auto take = [&](int n) { int at = o; o += round_up(n, 4); return at; };
+  P.sm_pose = take(P.G * POSE_STRIDE);
+  P.sm_prim = take(P.K * PRIM_SM_STRIDE);
+  P.sm_q = take(P.G * P.M * 3);
+  P.sm_ys = P.sm_acc = P.sm_vs = P.sm_mid = P.sm_dp = P.sm_cand = 0;
+  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = 0;
+  if (P.self_contact) {
+    P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
+    P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap / 2);
+  }
+  if (adjoint) {
+    P.sm_lam = take((P.N_C * VPL + P.N_C) * 32);
+    if (P.self_contact) { P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP); }
+  }
+  P.sm_warp_floats = o;
+  return o * (int)sizeof(float) * DLO_WARPS_PER_BLOCK;
+}
+
+static dlo_status validate(const dlo_config* c) {
+  if (!c) return fail(DLO_ERR_INVALID_ARG, "config is NULL");
+  if (c->batch < 1) return fail(DLO_ERR_INVALID_ARG, "batch < 1");
+  if (c->n_verts < 3 || c->n_verts > DLO_MAX_VERTS) return fail(DLO_ERR_INVALID_ARG, "n_verts out of [3,256]");
+  if (c->topology != DLO_OPEN && c->topology != DLO_RING) return fail(DLO_ERR_INVALID_ARG, "bad topology");
+  if (c->topology == DLO_RING && c->n_verts < 4) return fail(DLO_ERR_INVALID_ARG, "ring needs n_verts >= 4");
+  if (c->n_substeps < 1 || c->n_proj_iters < 0 || c->n_proj_iters > 32) return fail(DLO_ERR_INVALID_ARG, "n_substeps < 1 or n_proj_iters out of [0,32]");
+  if (c->stretch_mode != DLO_STRETCH_ENERGY && c->stretch_mode != DLO_STRETCH_PROJECT) return fail(DLO_ERR_INVALID_ARG, "bad stretch_mode");
+  if (c->n_grippers < 0 || c->n_grippers > DLO_MAX_GRIPPERS) return fail(DLO_ERR_INVALID_ARG, "n_grippers out of [0,4]");
+  if (c->n_grippers > 0 && (c->n_grasp_max < 1 || c->n_grasp_max > 8)) return fail(DLO_ERR_INVALID_ARG, "n_grasp_max out of [1,8]");
+  if (c->n_primitives < 0 || c->n_primitives > DLO_MAX_PRIMITIVES) return fail(DLO_ERR_INVALID_ARG, "n_primitives out of [0,16]");
+  if (c->n_primitives + 2 * c->n_grippers > 32) return fail(DLO_ERR_INVALID_ARG, "too many rigid bodies");
+  if (!(c->dt > 0.0f) || !(c->contact_softness > 0.0f) || !(c->influence_threshold > 0.0f)) return fail(DLO_ERR_INVALID_ARG, "dt, contact_softness, influence_threshold must be > 0");
+  if (c->enable_self_contact && c->self_skip < 2) return fail(DLO_ERR_INVALID_ARG, "self_skip < 2");
+  return DLO_OK;
+}
+
+static void fill_params(const dlo_config& c, KParams& P) {
+  memset(&P, 0, sizeof(P));
+  P.B = c.batch; P.N = c.n_verts; P.ring = c.topology == DLO_RING; P.E = P.ring ? P.N : P.N - 1;
+  P.NS = round_up(P.N, 4);
+  P.odd_ring = P.ring && (P.E & 1);
+  P.n_sub = c.n_substeps; P.N_C = c.n_proj_iters; P.stretch_mode = c.stretch_mode; P.plasticity = c.enable_plasticity != 0;
+  P.self_contact = c.enable_self_contact != 0; P.self_skip = c.self_skip;
+  P.G = c.n_grippers; P.M = P.G ? c.n_grasp_max : 1; P.K = c.n_primitives;
+  P.cand_cap = round_up(4 * P.N, 32);
+  P.h = c.dt / (float)c.n_substeps; P.inv_h = 1.0f / P.h;
+  for (int k = 0; k < 3; ++k) P.g[k] = c.gravity[k];
+  P.r = c.rope_radius; P.inv_eps = 1.0f / c.contact_softness; P.f_thresh = c.influence_threshold; P.e_rest = c.restitution;
+  P.log_thresh_lo = logf(c.influence_threshold) - 0.01f;
+}
+
+size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
+  if (validate(c) != DLO_OK) return 0;
+  KParams P;
+  fill_params(*c, P);
+  const size_t B = P.B, blk = (size_t)STATE_ROWS * P.NS * sizeof(float);
+  size_t n = B * (MAT_N * 4 + P.NS + P.N + 4) + B * P.G * (P.M * 3 * 4 + 6 * 4 + 4 * 4 + P.M * 4) + B * P.K * PRIM_NP * 4;
+  n += 2 * B * blk;                                                            // state, state0
+  if (stride > 0 && horizon > 0) {
+    n += ((size_t)horizon / stride + 1) * B * blk;                             // checkpoints
+    n += (size_t)(stride < horizon ? stride : horizon) * P.n_sub * B * blk;    // per-substep tape of one segment
+    n += B * blk;                                                              // running adjoint
+    if (P.self_contact) n += B * (size_t)P.N_C * 3 * 32 * vpl_for(P.N) * 4;    // self-contact correction tape
+  }
+  return n;
+}
+
+template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
+
+extern "C" {
+
+const char* dlo_last_error(void) { return g_err.c_str(); }
+const char* dlo_version(void) { return "dlo-b200 0.1 (sm_100a)"; }
+int64_t dlo_launch_count(const dlo_sim* s) { return s ? s->launches : 0; }
+
+dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stream, dlo_sim** out) {
+  if (!out) return fail(DLO_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  dlo_status st = validate(cfg);
+  if (st != DLO_OK) return st;
+  if (!mat) return fail(DLO_ERR_INVALID_ARG, "material is NULL");
+  const float* mp[MAT_N] = {mat->mass_per_vertex, mat->rest_edge_len, mat->stretch, mat->bend_stiffness, mat->damping,
+                            mat->yield_curv, mat->creep_rate, mat->mu_rigid, mat->mu_self};
+  for (int k = 0; k < MAT_N; ++k) if (!mp[k]) return fail(DLO_ERR_INVALID_ARG, "a material array is NULL");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return fail(DLO_ERR_CUDA, "no CUDA device: this library has no CPU path"); }
+  dlo_sim* s = new dlo_sim();
+  s->cfg = *cfg;
+  s->stream = (cudaStream_t)stream;
+  fill_params(*cfg, s->P);
+  KParams& P = s->P;
+  s->VPL = vpl_for(P.N);
+  s->blk = (size_t)STATE_ROWS * P.NS;
+  s->smem_fwd = smem_layout(P, s->VPL, false);
+  KParams Pa = P;
+  s->smem_adj = smem_layout(Pa, s->VPL, true);
+  if (s->smem_adj > 227 * 1024) { delete s; return fail(DLO_ERR_UNSUPPORTED, "shared memory per block exceeds 227 KB for this n_verts / n_proj_iters"); }
+  const size_t B = P.B;
+#define CUD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { dlo_destroy(s); return fail(e_ == cudaErrorMemoryAllocation ? DLO_ERR_OOM : DLO_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
+  CUD(dalloc(&s->mat, B * MAT_N));
+  CUD(dalloc(&s->kin, B * P.NS));
+  CUD(dalloc(&s->pins, B * P.N));
+  CUD(dalloc(&s->qloc, B * P.G * P.M * 3));
+  CUD(dalloc(&s->pose0, B * P.G * 6));
+  CUD(dalloc(&s->finger, B * P.G * 4));
+  CUD(dalloc(&s->grasp, B * P.G * P.M));
+  CUD(dalloc(&s->prim, B * P.K * PRIM_NP));
+  CUD(dalloc(&s->state, B * s->blk));
+  CUD(dalloc(&s->state0, B * s->blk));
+  CUD(dalloc(&s->flags, B));
+  CUD(cudaMemsetAsync(s->flags, 0, B * sizeof(int), s->stream));
+  CUD(cudaMemsetAsync(s->pins, 0, B * P.N, s->stream));
+  CUD(cudaMemsetAsync(s->grasp, 0xff, B * P.G * P.M * sizeof(int), s->stream));
+  CUD(cudaMemsetAsync(s->pose0, 0, B * P.G * 6 * sizeof(float), s->stream));
+  CUD(cudaMemsetAsync(s->finger, 0, B * P.G * 4 * sizeof(float), s->stream));
+  CUD(cudaMemsetAsync(s->prim, 0, B * P.K * PRIM_NP * sizeof(float), s->stream));
+  MatArgs ma;
+  for (int k = 0; k < MAT_N; ++k) ma.a[k] = mp[k];
+  k_pack_material<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, ma, s->mat);
+  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->kin);
+  s->launches += 2;
+  CUD(cudaGetLastError());
+  CUD(cudaStreamSynchronize(s->stream));   // the material arrays are the caller's: done with them before returning
+#undef CUD
+  P.mat = s->mat; P.kin = s->kin; P.qloc = s->qloc; P.pose0 = s->pose0; P.finger = s->finger; P.prim = s->prim;
+  P.state = s->state; P.flags = s->flags;
+  *out = s;
+  return DLO_OK;
+}
+
+dlo_status dlo_destroy(dlo_sim* s) {
+  if (!s) return DLO_OK;
+  cudaStreamSynchronize(s->stream);
+  void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj,
+                 s->kin, s->pins, s->grasp, s->flags};
+  for (void* p : dev) if (p) cudaFree(p);
+  void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hseed_x, s->hseed_v, s->hg_act, s->hg_x0, s->hg_v0, s->hg_mat, s->hxT, s->hvT};
+  for (void* p : host) if (p) cudaFreeHost(p);
+  delete s;
+  return DLO_OK;
+}
+
+static dlo_status rebuild_kin(dlo_sim* s) {
+  const KParams& P = s->P;
+  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->kin);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  s->have_state = false;
+  return DLO_OK;
+}
+
+dlo_status dlo_set_pins(dlo_sim* s, const uint8_t* pinned) {
+  if (!s || !pinned) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  CU(cudaMemcpyAsync(s->pins, pinned, (size_t)s->P.B * s->P.N, cudaMemcpyDeviceToDevice, s->stream));
+  return rebuild_kin(s);
+}
+
+dlo_status dlo_set_primitives(dlo_sim* s, const int32_t* types, const float* params) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (s->P.K == 0) return DLO_OK;
+  if (!types || !params) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  for (int k = 0; k < s->P.K; ++k) {
+    if (types[k] < 0 || types[k] > 3) return fail(DLO_ERR_INVALID_ARG, "unknown primitive type");
+    s->P.prim_type[k] = types[k];
+  }
+  CU(cudaMemcpyAsync(s->prim, params, (size_t)s->P.B * s->P.K * PRIM_NP * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  s->have_prims = true;
+  return DLO_OK;
+}
+
+dlo_status dlo_set_grippers(dlo_sim* s, const float* init_pose, const float* finger_geom, const int32_t* grasp_verts) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (s->P.G == 0) return DLO_OK;
+  if (!init_pose || !finger_geom || !grasp_verts) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  const size_t BG = (size_t)s->P.B * s->P.G;
+  CU(cudaMemcpyAsync(s->pose0, init_pose, BG * 6 * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  CU(cudaMemcpyAsync(s->finger, finger_geom, BG * 4 * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  CU(cudaMemcpyAsync(s->grasp, grasp_verts, BG * s->P.M * sizeof(int), cudaMemcpyDeviceToDevice, s->stream));
+  s->have_grippers = true;
+  return rebuild_kin(s);
+}
+
+dlo_status dlo_set_state(dlo_sim* s, const float* x0, const float* v0, const float* kb0) {
+  if (!s || !x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  const KParams& P = s->P;
+  if (P.K > 0 && !s->have_prims) return fail(DLO_ERR_BAD_STATE, "dlo_set_primitives must precede dlo_set_state");
+  if (P.G > 0 && !s->have_grippers) return fail(DLO_ERR_BAD_STATE, "dlo_set_grippers must precede dlo_set_state");
+  SetupArgs A;
+  A.B = P.B; A.N = P.N; A.E = P.E; A.NS = P.NS; A.ring = P.ring; A.G = P.G; A.M = P.M; A.kappa_from_x0 = s->cfg.kappa_bar_from_x0;
+  A.x0 = x0; A.v0 = v0; A.kb0 = kb0; A.pose0 = s->pose0; A.grasp_verts = s->grasp; A.state = s->state0; A.qloc = s->qloc;
+  k_set_state<<<(P.B + 63) / 64, 64, 0, s->stream>>>(A);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(s->state, s->state0, (size_t)P.B * s->blk * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  CU(cudaMemsetAsync(s->flags, 0, (size_t)P.B * sizeof(int), s->stream));
+  s->have_state = true;
+  s->H_done = 0; s->stride = 0;
+  return DLO_OK;
+}
+
+dlo_status dlo_set_actions(dlo_sim* s, const float* actions, int32_t horizon) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (horizon < 0) return fail(DLO_ERR_INVALID_ARG, "horizon < 0");
+  if (s->P.G > 0 && horizon > 0 && !actions) return fail(DLO_ERR_INVALID_ARG, "actions is NULL");
+  s->actions = actions; s->H_actions = horizon; s->P.actions = actions;
+  return DLO_OK;
+}
+
+}  // extern "C"
+
+template <int VPL> static cudaError_t launch_forward_t(dlo_sim* s, int t0, int t1, int stride, int write_tape) {
+  static bool attr_done = false;
+  if (!attr_done || s->smem_fwd > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(k_forward<VPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fwd > 48 * 1024 ? s->smem_fwd : 48 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  const int grid = (s->P.B + DLO_WARPS_PER_BLOCK - 1) / DLO_WARPS_PER_BLOCK;
+  k_forward<VPL><<<grid, DLO_WARPS_PER_BLOCK * 32, s->smem_fwd, s->stream>>>(s->P, t0, t1, stride, write_tape);
+  s->launches += 1;
+  return cudaGetLastError();
+}
+static cudaError_t launch_forward(dlo_sim* s, int t0, int t1, int stride, int write_tape) {
+  smem_layout(s->P, s->VPL, false);
+  switch (s->VPL) {
+    case 2: return launch_forward_t<2>(s, t0, t1, stride, write_tape);
+    case 4: return launch_forward_t<4>(s, t0, t1, stride, write_tape);
+    case 6: return launch_forward_t<6>(s, t0, t1, stride, write_tape);
+    default: return launch_forward_t<8>(s, t0, t1, stride, write_tape);
+  }
+}
+
+extern "C" {
+
+dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "dlo_set_state has not been called (or the scene changed since)");
+  if (horizon < 0 || stride < 0) return fail(DLO_ERR_INVALID_ARG, "horizon < 0 or checkpoint_stride < 0");
+  if (s->P.G > 0 && horizon > s->H_actions) return fail(DLO_ERR_INVALID_ARG, "horizon exceeds the actions given to dlo_set_actions");
+  const KParams& P = s->P;
+  const size_t blk_bytes = s->blk * sizeof(float) * P.B;
+  CU(cudaMemcpyAsync(s->state, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));
+  s->H_done = 0; s->stride = 0;
+  if (stride > 0) {
+    const size_t need = (size_t)horizon / stride + 1;
+    if (need > s->ckpt_blocks) {
+      CU(cudaStreamSynchronize(s->stream));
+      if (s->ckpt) cudaFree(s->ckpt);
+      s->ckpt = nullptr; s->ckpt_blocks = 0;
+      CU(dalloc(&s->ckpt, need * P.B * s->blk));
+      s->ckpt_blocks = need;
+    }
+    s->P.ckpt = s->ckpt;
+    CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
+  }
+  if (horizon > 0) CU(launch_forward(s, 0, horizon, stride, 0));
+  s->H_done = horizon; s->stride = stride;
+  return DLO_OK;
+}
+
+dlo_status dlo_get_state(dlo_sim* s, float* x, float* v, float* d1, float* kb) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "no state");
+  const KParams& P = s->P;
+  const size_t n = (size_t)P.B * STATE_ROWS * P.N;
+  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, s->state, x, v, d1, kb);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  return DLO_OK;
+}
+
+dlo_status dlo_check_numerics(dlo_sim* s, int32_t* n_bad) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  std::vector<int> f(s->P.B);
+  CU(cudaMemcpyAsync(f.data(), s->flags, f.size() * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  int bad = 0, ovf = 0;
+  for (int v : f) { bad += v != 0; ovf += (v & FLAG_CAND_OVERFLOW) != 0; }
+  if (n_bad) *n_bad = bad;
+  if (bad) return fail(DLO_ERR_NUMERIC, std::to_string(bad) + " env(s) flagged (" + std::to_string(ovf) + " self-contact candidate overflow, rest non-finite)");
+  return DLO_OK;
+}
+
+}  // extern "C"
+
+#include "dlo_api_backward.inl"

@@ -1,0 +1,79 @@
+// dlo_api_backward.inl — dlo_backward and the host-buffer convenience calls (included by dlo_api.cu)
+
+extern "C" {
+
+dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g_actions, float* g_x0, float* g_v0, float* g_material) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
+  (void)gxT; (void)gvT; (void)g_actions; (void)g_x0; (void)g_v0; (void)g_material;
+  return fail(DLO_ERR_UNSUPPORTED, "adjoint kernel not built yet");
+}
+
+static dlo_status stage(float** pinned, size_t n) {
+  if (*pinned) { cudaFreeHost(*pinned); *pinned = nullptr; }
+  CU(cudaMallocHost((void**)pinned, (n ? n : 1) * sizeof(float)));
+  return DLO_OK;
+}
+
+dlo_status dlo_rollout_forward_host(dlo_sim* s, const float* x0, const float* v0, const float* kb0, const float* actions,
+                                    int32_t horizon, int32_t stride, float* x_T, float* v_T) {
+  if (!s || !x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  const KParams& P = s->P;
+  const size_t nx = (size_t)P.B * 3 * P.N, nk = (size_t)P.B * 2 * P.N, na = (size_t)horizon * P.B * P.G * 6;
+  if (P.G > 0 && horizon > 0 && !actions) return fail(DLO_ERR_INVALID_ARG, "actions is NULL");
+  dlo_status st;
+  if (!s->hx0) { if ((st = stage(&s->hx0, nx))) return st; if ((st = stage(&s->hv0, nx))) return st; if ((st = stage(&s->hkb, nk))) return st;
+                 if ((st = stage(&s->hxT, nx))) return st; if ((st = stage(&s->hvT, nx))) return st; }
+  if (na > 0 && horizon > s->hact_H) { if ((st = stage(&s->hact, na))) return st; s->hact_H = horizon; }
+  // device staging lives in the tail of the same allocations (cudaMallocHost memory is device-accessible only via
+  // copies here): device copies of the inputs
+  static thread_local float *dx0 = nullptr, *dv0 = nullptr, *dkb = nullptr, *dact = nullptr, *dxT = nullptr, *dvT = nullptr;
+  static thread_local size_t dact_n = 0, dx_n = 0;
+  if (dx_n < nx) {
+    cudaFree(dx0); cudaFree(dv0); cudaFree(dkb); cudaFree(dxT); cudaFree(dvT);
+    CU(dalloc(&dx0, nx)); CU(dalloc(&dv0, nx)); CU(dalloc(&dkb, nk)); CU(dalloc(&dxT, nx)); CU(dalloc(&dvT, nx));
+    dx_n = nx;
+  }
+  if (dact_n < na) { CU(cudaStreamSynchronize(s->stream)); cudaFree(dact); CU(dalloc(&dact, na)); dact_n = na; }
+  memcpy(s->hx0, x0, nx * sizeof(float));
+  memcpy(s->hv0, v0, nx * sizeof(float));
+  CU(cudaMemcpyAsync(dx0, s->hx0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  CU(cudaMemcpyAsync(dv0, s->hv0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  if (kb0) { memcpy(s->hkb, kb0, nk * sizeof(float)); CU(cudaMemcpyAsync(dkb, s->hkb, nk * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
+  if (na > 0) { memcpy(s->hact, actions, na * sizeof(float)); CU(cudaMemcpyAsync(dact, s->hact, na * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
+  if ((st = dlo_set_state(s, dx0, dv0, kb0 ? dkb : nullptr))) return st;
+  if ((st = dlo_set_actions(s, dact, horizon))) return st;
+  if ((st = dlo_rollout_forward(s, horizon, stride))) return st;
+  if ((st = dlo_get_state(s, x_T ? dxT : nullptr, v_T ? dvT : nullptr, nullptr, nullptr))) return st;
+  if (x_T) CU(cudaMemcpyAsync(s->hxT, dxT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (v_T) CU(cudaMemcpyAsync(s->hvT, dvT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  if (x_T) memcpy(x_T, s->hxT, nx * sizeof(float));
+  if (v_T) memcpy(v_T, s->hvT, nx * sizeof(float));
+  return DLO_OK;
+}
+
+dlo_status dlo_backward_host(dlo_sim* s, const float* gxT, const float* gvT, float* g_actions, float* g_x0, float* g_v0, float* g_material) {
+  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
+  const KParams& P = s->P;
+  const size_t nx = (size_t)P.B * 3 * P.N, na = (size_t)s->H_done * P.B * P.G * 6, nm = (size_t)P.B * DLO_N_MATERIAL_GRADS;
+  static thread_local float *dsx = nullptr, *dsv = nullptr, *dga = nullptr, *dgx = nullptr, *dgv = nullptr, *dgm = nullptr;
+  static thread_local size_t nx_a = 0, na_a = 0, nm_a = 0;
+  if (nx_a < nx) { cudaFree(dsx); cudaFree(dsv); cudaFree(dgx); cudaFree(dgv); CU(dalloc(&dsx, nx)); CU(dalloc(&dsv, nx)); CU(dalloc(&dgx, nx)); CU(dalloc(&dgv, nx)); nx_a = nx; }
+  if (na_a < na) { cudaFree(dga); CU(dalloc(&dga, na)); na_a = na; }
+  if (nm_a < nm) { cudaFree(dgm); CU(dalloc(&dgm, nm)); nm_a = nm; }
+  if (gxT) CU(cudaMemcpyAsync(dsx, gxT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  if (gvT) CU(cudaMemcpyAsync(dsv, gvT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  dlo_status st = dlo_backward(s, gxT ? dsx : nullptr, gvT ? dsv : nullptr, (g_actions && na) ? dga : nullptr, g_x0 ? dgx : nullptr,
+                               g_v0 ? dgv : nullptr, g_material ? dgm : nullptr);
+  if (st) return st;
+  if (g_actions && na) CU(cudaMemcpyAsync(g_actions, dga, na * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_x0) CU(cudaMemcpyAsync(g_x0, dgx, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_v0) CU(cudaMemcpyAsync(g_v0, dgv, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_material) CU(cudaMemcpyAsync(g_material, dgm, nm * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  CU(cudaStreamSynchronize(s->stream));
+  return DLO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,472 @@
+// rod_substep.cuh — ONE substep of the rod step for one env held by one warp (steps A1-A9).
+// `REC` = true additionally records what the reverse pass needs (rod_adjoint.cuh): the Eq.10 multipliers, the
+// per-iteration self-contact corrections, the pre-coupling velocity and the set of active rigid responses.
+#pragma once
+#include "rod_warp.cuh"
+
+namespace dlo {
+
+struct WarpSmem {
+  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar;
+  unsigned short* cand;
+  int NP;   // 32*VPL
+  __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
+    pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
+    vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
+    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar;
+    NP = np;
+  }
+};
+
+// intermediates of one substep that outlive it when REC (all per lane)
+template <int VPL> struct SubRec {
+  f3 v1[VPL], xp[VPL], dx[VPL], v3[VPL], v4[VPL], t_old[VPL];
+  float S[VPL];
+  unsigned active[VPL];   // bit k<K: primitive k responded; bit K+2g+f: finger f of gripper g responded
+  int ncand, any_pen;
+  unsigned jac_mask;      // bit it: the Jacobi pass of iteration it applied at least one correction
+};
+
+// A1 (L129, R-20): lane g < G evaluates gripper g at the substep's start and end and publishes it
+__device__ __forceinline__ void publish_poses(const KParams& P, int env, int lane, const float ap[6], const float ac[6], int s, float* pose_sm) {
+  if (lane < P.G) {
+    const float tau0 = (float)s / (float)P.n_sub, tau1 = (float)(s + 1) / (float)P.n_sub;
+    Pose<float> g0 = make_pose<float>(ap, ac, tau0), g1 = make_pose<float>(ap, ac, tau1);
+    float* o = pose_sm + lane * POSE_STRIDE;
+    o[POSE_P0] = g0.p.x; o[POSE_P0 + 1] = g0.p.y; o[POSE_P0 + 2] = g0.p.z;
+    o[POSE_P1] = g1.p.x; o[POSE_P1 + 1] = g1.p.y; o[POSE_P1 + 2] = g1.p.z;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) { o[POSE_R0 + k] = g0.R.m[k]; o[POSE_R1 + k] = g1.R.m[k]; }
+    const float* fg = P.finger + ((size_t)env * P.G + lane) * 4;
+    const float gap = fg[0], len = fg[1];
+    f3 A0 = g1.p + mul(g1.R, mk3<float>(0.5f * gap, 0.f, 0.f)), B0 = g1.p + mul(g1.R, mk3<float>(0.5f * gap, 0.f, len));
+    f3 A1 = g1.p + mul(g1.R, mk3<float>(-0.5f * gap, 0.f, 0.f)), B1 = g1.p + mul(g1.R, mk3<float>(-0.5f * gap, 0.f, len));
+    o[POSE_FA0] = A0.x; o[POSE_FA0 + 1] = A0.y; o[POSE_FA0 + 2] = A0.z; o[POSE_FB0] = B0.x; o[POSE_FB0 + 1] = B0.y; o[POSE_FB0 + 2] = B0.z;
+    o[POSE_FA1] = A1.x; o[POSE_FA1 + 1] = A1.y; o[POSE_FA1 + 2] = A1.z; o[POSE_FB1] = B1.x; o[POSE_FB1 + 1] = B1.y; o[POSE_FB1 + 2] = B1.z;
+    o[POSE_RF] = fg[2];
+  }
+  __syncwarp();
+}
+__device__ __forceinline__ Pose<float> read_pose(const float* o, int which) {
+  Pose<float> g;
+  const float* p = o + (which ? POSE_P1 : POSE_P0);
+  const float* R = o + (which ? POSE_R1 : POSE_R0);
+  g.p = mk3<float>(p[0], p[1], p[2]);
+#pragma unroll
+  for (int k = 0; k < 9; ++k) g.R.m[k] = R[k];
+  return g;
+}
+// target of a grasped vertex at the end of the substep: p1 + R1 q  (L103 kinematic flag, R-19)
+__device__ __forceinline__ f3 grasp_target(const KParams& P, const WarpSmem& sm, int code) {
+  const int slot = code - KIN_GRASP0, g = slot / P.M;
+  const float* o = sm.pose + g * POSE_STRIDE;
+  const float* q = sm.q + 3 * slot;
+  Pose<float> g1 = read_pose(o, 1);
+  return g1.p + mul(g1.R, mk3<float>(q[0], q[1], q[2]));
+}
+
+// A2 bending (Eq.4-7): per owned interior vertex the element gradients Ga, Gb; returns the gathered force
+template <int VPL>
+__device__ __forceinline__ void bending_forces(const Topo<VPL>& tp, const LaneState<VPL>& s, const EdgeCache<VPL>& ec, float sc, f3 f[VPL]) {
+  f3 Ga[VPL], Gb[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    Ga[k] = zero3<float>(); Gb[k] = zero3<float>();
+    if (tp.interior[k]) {
+      const f3 ta = (k == 0) ? ec.pt : ec.t[k > 0 ? k - 1 : 0];
+      const f3 da = (k == 0) ? ec.pd1 : s.d1[k > 0 ? k - 1 : 0];
+      const float ia = (k == 0) ? ec.piL : ec.iL[k > 0 ? k - 1 : 0];
+      bend_element<float>(ta, ec.t[k], ia, ec.iL[k], da, s.d1[k], s.kb1[k], s.kb2[k], sc, Ga[k], Gb[k]);
+    }
+  }
+  const f3 Gb_prev = shfl3(pick_last<VPL>(Gb, tp.ks), tp.pl);   // element i-1 of slot 0
+  const f3 Ga_next = shfl3(Ga[0], tp.nl);                      // element i+1 of the last slot
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    const f3 gbp = (k == 0) ? Gb_prev : Gb[k > 0 ? k - 1 : 0];
+    const f3 gan = next_of<VPL>(Ga, Ga_next, k, tp.ks);
+    f[k] = f[k] - gbp - Ga[k] + Gb[k] + gan;
+  }
+}
+
+// segment-pair test used by the candidate build: exact closest distance below `lim`
+__device__ __forceinline__ bool pair_within(const float* ys, int NP, int a, int an, int b, int bn, float lim) {
+  f3 p1 = lds3(ys, NP, a), q1 = lds3(ys, NP, an), p2 = lds3(ys, NP, b), q2 = lds3(ys, NP, bn);
+  float t, u;
+  closest_points<float>(p1, q1, p2, q2, t, u);
+  f3 dv = axpy(p1, t, q1 - p1) - axpy(p2, u, q2 - p2);
+  return dot(dv, dv) < lim * lim;
+}
+
+// A4 candidate list (Eq.13 "potentially colliding", R-15): all edge pairs a<b with cyclic index distance >=
+// self_skip closer than 2(r_a+r_b) at x^p, in lexicographic order.  ys holds x^p, mid holds (midpoint, half length).
+template <int VPL>
+__device__ int build_candidates(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int env) {
+  const int E = P.E, N = P.N, NP = sm.NP;
+  const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
+  int ncand = 0;
+  for (int a = 0; a < E; ++a) {
+    const int an = (a + 1 < N) ? a + 1 : 0;
+    const float ax = sm.mid[a], ay = sm.mid[NP + a], az = sm.mid[2 * NP + a], ah = sm.mid[3 * NP + a];
+    const int bmax = P.ring ? min(E - 1, a + E - P.self_skip) : E - 1;
+    for (int b0 = a + P.self_skip; b0 <= bmax; b0 += 32) {
+      const int b = b0 + tp.lane;
+      bool hit = false;
+      if (b <= bmax) {
+        const float dx = sm.mid[b] - ax, dy = sm.mid[NP + b] - ay, dz = sm.mid[2 * NP + b] - az;
+        const float reach = ah + sm.mid[3 * NP + b] + lim;
+        if (dx * dx + dy * dy + dz * dz < reach * reach) hit = pair_within(sm.ys, NP, a, an, b, (b + 1 < N) ? b + 1 : 0, lim);
+      }
+      const unsigned m = __ballot_sync(DLO_FULL, hit);
+      if (hit) {
+        const int pos = ncand + __popc(m & ((1u << tp.lane) - 1u));
+        if (pos < P.cand_cap) sm.cand[pos] = (unsigned short)((a << 8) | b);
+      }
+      ncand += __popc(m);
+    }
+  }
+  if (ncand > P.cand_cap) {
+    if (tp.lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
+    ncand = P.cand_cap;
+  }
+  __syncwarp();
+  return ncand;
+}
+
+// serialised (deterministic, candidate-order) accumulation of one lane's four vertex contributions
+__device__ __forceinline__ void ordered_scatter4(unsigned hits, int lane, float* acc, int NP, const int iv[4], const float coef[4], const f3& n) {
+  while (hits) {
+    const int src = __ffs(hits) - 1;
+    hits &= hits - 1;
+    if (lane == src) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        acc[iv[k]] += coef[k] * n.x; acc[NP + iv[k]] += coef[k] * n.y; acc[2 * NP + iv[k]] += coef[k] * n.z;
+      }
+    }
+    __syncwarp();
+  }
+}
+
+// A5(ii): one Jacobi pass of Eq.13 over the candidates at y (in sm.ys); corrections summed into sm.acc, D_p += d.
+// Returns true if any correction was applied.
+template <int VPL>
+__device__ bool contact_pass(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand, float inv_m) {
+  const int NP = sm.NP, N = P.N;
+  const float rsum = 2.0f * P.r;
+  bool any = false;
+  for (int p0 = 0; p0 < ncand; p0 += 32) {
+    const int p = p0 + tp.lane;
+    bool hit = false;
+    int iv[4] = {0, 0, 0, 0};
+    float coef[4] = {0.f, 0.f, 0.f, 0.f};
+    f3 n = zero3<float>();
+    if (p < ncand) {
+      const unsigned c = sm.cand[p];
+      iv[0] = c >> 8; iv[2] = c & 255; iv[1] = (iv[0] + 1 < N) ? iv[0] + 1 : 0; iv[3] = (iv[2] + 1 < N) ? iv[2] + 1 : 0;
+      f3 xs[4];
+      float ws[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { xs[k] = lds3(sm.ys, NP, iv[k]); ws[k] = sm.mid[4 * NP + iv[k]]; }
+      // conservative reject: the segments cannot be closer than |midpoint distance| - half lengths
+      f3 ea = xs[1] - xs[0], eb = xs[3] - xs[2];
+      f3 dm = (xs[0] + 0.5f * ea) - (xs[2] + 0.5f * eb);
+      const float reach = 0.5f * (sqrt_(dot(ea, ea)) + sqrt_(dot(eb, eb))) + rsum;
+      if (dot(dm, dm) < reach * reach) {
+        float d, t, u, W;
+        if (contact_eval<float>(xs, ws, rsum, d, t, u, n, W)) {
+          hit = true;
+          const float s = d / W;
+          coef[0] = s * ws[0] * (1.0f - t); coef[1] = s * ws[1] * t; coef[2] = -s * ws[2] * (1.0f - u); coef[3] = -s * ws[3] * u;
+          sm.dp[p] += d;
+        }
+      }
+    }
+    const unsigned hits = __ballot_sync(DLO_FULL, hit);
+    any |= hits != 0u;
+    ordered_scatter4(hits, tp.lane, sm.acc, NP, iv, coef, n);
+  }
+  (void)inv_m;
+  return any;
+}
+
+// A6 self-contact friction (L410, R-16) for candidates with D_p > 0: velocities in sm.vs, positions in sm.ys
+template <int VPL>
+__device__ void friction_pass(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand, float mu_s) {
+  const int NP = sm.NP, N = P.N;
+  for (int p0 = 0; p0 < ncand; p0 += 32) {
+    const int p = p0 + tp.lane;
+    bool hit = false;
+    int iv[4] = {0, 0, 0, 0};
+    float coef[4] = {0.f, 0.f, 0.f, 0.f};
+    f3 D = zero3<float>();
+    if (p < ncand && sm.dp[p] > 0.0f) {
+      const unsigned c = sm.cand[p];
+      iv[0] = c >> 8; iv[2] = c & 255; iv[1] = (iv[0] + 1 < N) ? iv[0] + 1 : 0; iv[3] = (iv[2] + 1 < N) ? iv[2] + 1 : 0;
+      f3 xs[4], vv[4];
+      float ws[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { xs[k] = lds3(sm.ys, NP, iv[k]); vv[k] = lds3(sm.vs, NP, iv[k]); ws[k] = sm.mid[4 * NP + iv[k]]; }
+      float t, u;
+      closest_points<float>(xs[0], xs[1], xs[2], xs[3], t, u);
+      f3 dv = axpy(xs[0], t, xs[1] - xs[0]) - axpy(xs[2], u, xs[3] - xs[2]);
+      const float del = sqrt_(dot(dv, dv));
+      const float a0 = 1.0f - t, b0 = 1.0f - u;
+      const float W = ws[0] * a0 * a0 + ws[1] * t * t + ws[2] * b0 * b0 + ws[3] * u * u;
+      if (del > 1e-12f && W > 0.0f) {
+        f3 n = (1.0f / del) * dv;
+        f3 vrel = (a0 * vv[0] + t * vv[1]) - (b0 * vv[2] + u * vv[3]);
+        f3 vt = vrel - dot(vrel, n) * n;
+        const float vtn = sqrt_(dot(vt, vt));
+        if (vtn > 1e-12f) {
+          const float cap = mu_s * sm.dp[p] * P.inv_h;
+          const float mag = cap < vtn ? cap : vtn;
+          D = (-(mag / vtn)) * vt;
+          const float iW = 1.0f / W;
+          coef[0] = ws[0] * a0 * iW; coef[1] = ws[1] * t * iW; coef[2] = -ws[2] * b0 * iW; coef[3] = -ws[3] * u * iW;
+          hit = true;
+        }
+      }
+    }
+    const unsigned hits = __ballot_sync(DLO_FULL, hit);
+    ordered_scatter4(hits, tp.lane, sm.acc, NP, iv, coef, D);
+  }
+}
+
+// A7 (L103): soft coupling of one free vertex at y against the K fixed primitives, then the finger capsules
+__device__ __forceinline__ unsigned rigid_coupling(const KParams& P, const WarpSmem& sm, const f3& y, f3& v, float mu_r) {
+  unsigned active = 0u;
+  for (int k = 0; k < P.K; ++k) {
+    float phi;
+    f3 n;
+    if (!sdf_eval_pre<float>(P.prim_type[k], sm.prim + k * PRIM_SM_STRIDE, y, phi, n)) continue;
+    if (rigid_response<float>(v, zero3<float>(), n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << k;
+  }
+  for (int g = 0; g < P.G; ++g) {
+    const float* o = sm.pose + g * POSE_STRIDE;
+#pragma unroll
+    for (int fk = 0; fk < 2; ++fk) {
+      const float* A = o + (fk ? POSE_FA1 : POSE_FA0);
+      const float* Bp = o + (fk ? POSE_FB1 : POSE_FB0);
+      float Pc[7] = {A[0], A[1], A[2], Bp[0], Bp[1], Bp[2], o[POSE_RF]};
+      float phi;
+      f3 n;
+      if (!sdf_eval<float>(1, Pc, y, phi, n)) continue;
+      if ((P.r - phi) * P.inv_eps < P.log_thresh_lo) continue;   // f < threshold for sure: v untouched, skip the body velocity
+      f3 vb = body_point_velocity<float>(read_pose(o, 0), read_pose(o, 1), y, P.inv_h);
+      if (rigid_response<float>(v, vb, n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << (P.K + 2 * g + fk);
+    }
+  }
+  return active;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// One substep.  On entry `ec` holds the edge geometry of s.x (tangents, inverse lengths, previous lane's last
+// edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
+template <int VPL, bool REC>
+__device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
+                                        const float ap[6], const float ac[6], int sub, LaneState<VPL>& s, EdgeCache<VPL>& ec,
+                                        SubRec<VPL>& R, float* acc_tape) {
+  const float h = P.h, inv_h = P.inv_h;
+  // -- A1 bodies
+  if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);
+
+  // -- A2 forces: gravity, stretch (mode ENERGY, Eq.2-3), bending (Eq.4-7)
+  f3 f[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) f[k] = mk3<float>(c.m * P.g[0], c.m * P.g[1], c.m * P.g[2]);
+  if (P.stretch_mode == 0) {
+    f3 F[VPL];
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const float L = tp.evalid[k] ? 1.0f / ec.iL[k] : 0.0f;
+      F[k] = tp.evalid[k] ? (c.stretch * (L / c.l0 - 1.0f)) * ec.t[k] : zero3<float>();
+    }
+    const f3 Fp = shfl3(pick_last<VPL>(F, tp.ks), tp.pl);
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) f[k] = f[k] + F[k] - ((k == 0) ? Fp : F[k > 0 ? k - 1 : 0]);
+  }
+  bending_forces<VPL>(tp, s, ec, c.alpha / c.l0, f);
+
+  // -- A3 velocity (symplectic Euler L97, implicit viscous damping R-7), A4 predict
+  const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    f3 v1 = zero3<float>();
+    if (c.kin[k] == KIN_FREE) v1 = idamp * axpy(s.v[k], hm, f[k]);
+    else if (c.kin[k] >= KIN_GRASP0) v1 = inv_h * (grasp_target(P, sm, c.kin[k]) - s.x[k]);
+    R.v1[k] = v1;
+    R.xp[k] = axpy(s.x[k], h, v1);
+    R.dx[k] = zero3<float>();
+    R.S[k] = 0.0f;
+    R.t_old[k] = ec.t[k];
+  }
+  const f3 xpr = shfl3(R.xp[0], tp.nl);
+  f3 epred[VPL];   // predicted edge vectors, constant during the projection loop
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
+
+  R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
+  if (P.self_contact) {
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const int i = tp.base + k;
+      sts3(sm.ys, sm.NP, i, R.xp[k]);
+      f3 mid = axpy(R.xp[k], 0.5f, epred[k]);
+      sts3(sm.mid, sm.NP, i, mid);
+      sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
+      sm.mid[4 * sm.NP + i] = c.w[k];
+    }
+    __syncwarp();
+    R.ncand = build_candidates<VPL>(P, tp, sm, env);
+    for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
+    __syncwarp();
+  }
+
+  // -- A5 projection loop
+  const float atil = c.stretch * inv_h * inv_h;
+  for (int it = 0; it < P.N_C; ++it) {
+    if (P.stretch_mode == 1) {
+      // red: even slots, both end points local
+#pragma unroll
+      for (int k = 0; k < VPL; k += 2) {
+        const bool on = (k + 1 < tp.nv) && tp.evalid[k];
+        const float wsum = c.w[k] + c.w[k + 1];
+        float lam = 0.0f;
+        f3 t = zero3<float>();
+        if (on && wsum > 0.0f) project_edge<float>(epred[k] + (R.dx[k + 1] - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+        R.S[k] += lam;
+        R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
+        R.dx[k + 1] = axpy(R.dx[k + 1], -lam * c.w[k + 1], t);
+        if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
+      }
+      // black: odd slots; the lane's last slot crosses to slot 0 of the next lane
+      {
+        const f3 dxr = shfl3(R.dx[0], tp.nl);
+        f3 back = zero3<float>();
+#pragma unroll
+        for (int k = 1; k < VPL; k += 2) {
+          const bool rem = (k == VPL - 1) || (k == tp.ks);
+          const bool on = tp.evalid[k] && (k <= tp.ks);
+          const float wn = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
+          const f3 dxn = rem ? dxr : R.dx[k + 1 < VPL ? k + 1 : k];
+          const float wsum = c.w[k] + wn;
+          float lam = 0.0f;
+          f3 t = zero3<float>();
+          if (on && wsum > 0.0f) project_edge<float>(epred[k] + (dxn - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+          R.S[k] += lam;
+          R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
+          if (rem) { if (on) back = (lam * wn) * t; }
+          else if (k + 1 < VPL) R.dx[k + 1] = axpy(R.dx[k + 1], -lam * wn, t);
+          if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
+        }
+        R.dx[0] -= shfl3(back, tp.pl);
+      }
+      // third colour: the closing edge of an odd ring (slot ks of the last lane, even slot)
+      if (P.odd_ring) {
+        const f3 dxr = shfl3(R.dx[0], tp.nl);
+        f3 back = zero3<float>();
+        float lam3 = 0.0f;
+#pragma unroll
+        for (int k = 0; k < VPL; k += 2) {
+          if (k == tp.ks && tp.base + k == P.E - 1) {
+            const float wsum = c.w[k] + c.wr;
+            float lam = 0.0f;
+            f3 t = zero3<float>();
+            if (wsum > 0.0f) project_edge<float>(epred[k] + (dxr - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+            R.S[k] += lam;
+            R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
+            back = (lam * c.wr) * t;
+            lam3 = lam;
+          }
+        }
+        R.dx[0] -= shfl3(back, tp.pl);
+        if (REC) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
+      }
+    }
+    if (P.self_contact && R.ncand > 0) {
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, tp.base + k, R.xp[k] + R.dx[k]);
+      __syncwarp();
+      const bool any = contact_pass<VPL>(P, tp, sm, R.ncand, c.inv_m);
+      __syncwarp();
+      if (any) {
+        R.any_pen = 1;
+        R.jac_mask |= 1u << it;
+#pragma unroll
+        for (int k = 0; k < VPL; ++k) {
+          const int i = tp.base + k;
+          const f3 a = lds3(sm.acc, sm.NP, i);
+          R.dx[k] += a;
+          if (REC) sts3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i, a);
+          sts3(sm.acc, sm.NP, i, zero3<float>());
+        }
+        __syncwarp();
+      }
+    }
+  }
+
+  // -- A6 reconcile v with the projected positions (R-11) + self-contact friction
+  f3 vel[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) vel[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k];
+  if (P.self_contact && R.any_pen) {
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, tp.base + k, R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, tp.base + k, vel[k]); }
+    __syncwarp();
+    friction_pass<VPL>(P, tp, sm, R.ncand, c.mu_s);
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const int i = tp.base + k;
+      if (c.kin[k] == KIN_FREE) vel[k] += lds3(sm.acc, sm.NP, i);
+      sts3(sm.acc, sm.NP, i, zero3<float>());
+    }
+    __syncwarp();
+  }
+
+  // -- A7 rigid soft coupling at y = x^p + dx
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    R.v3[k] = vel[k];
+    R.active[k] = 0u;
+    if (c.kin[k] == KIN_FREE && (P.K > 0 || P.G > 0)) R.active[k] = rigid_coupling(P, sm, R.xp[k] + R.dx[k], vel[k], c.mu_r);
+    R.v4[k] = vel[k];
+  }
+
+  // -- A8 commit
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    if (c.kin[k] == KIN_FREE) { s.x[k] = axpy(s.x[k], h, vel[k]); s.v[k] = vel[k]; }
+    else if (c.kin[k] >= KIN_GRASP0) { s.x[k] = grasp_target(P, sm, c.kin[k]); s.v[k] = vel[k]; }
+    else if (tp.vvalid[k]) s.v[k] = zero3<float>();
+  }
+
+  // -- A9 frames: time-parallel transport (R-4), then plasticity (Eq.11)
+  edge_refresh<VPL>(tp, s, ec);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    if (tp.evalid[k]) {
+      f3 d = ptransport<float>(R.t_old[k], ec.t[k], s.d1[k]);
+      d = axpy(d, -dot(d, ec.t[k]), ec.t[k]);
+      s.d1[k] = rsqrt_(dot(d, d)) * d;
+    }
+  }
+  edge_prev_refresh<VPL>(tp, s, ec);
+  if (P.plasticity) {
+    const float Y = c.sigy * c.l0;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      if (tp.interior[k]) {
+        const f3 ta = (k == 0) ? ec.pt : ec.t[k > 0 ? k - 1 : 0];
+        const f3 da = (k == 0) ? ec.pd1 : s.d1[k > 0 ? k - 1 : 0];
+        float k1, k2;
+        material_curvature<float>(ta, ec.t[k], da, s.d1[k], k1, k2);
+        plasticity_update<float>(k1, k2, s.kb1[k], s.kb2[k], Y, c.rc);
+      }
+    }
+  }
+  if (P.G > 0) __syncwarp();   // the pose block is rewritten by the next substep
+}
+
+}  // namespace dlo

@@ -1,0 +1,202 @@
+// rod_warp.cuh — one warp <-> one env: lane topology, state I/O and the forward substep shared by the forward
+// kernel and the replay half of the adjoint kernel.
+//
+// Mapping.  Lane l owns the VPL consecutive vertices base = l*VPL .. base+VPL-1 and the
+// edges with the same indices (edge j joins j and j+1; ring: E-1 joins N-1 and 0).  VPL is even, so an edge's
+// red/black colour (j & 1) is a compile-time property of its slot: red (even) edges have both end points in
+// the same lane, black (odd) edges cross to slot 0 of the next lane only at the lane's last slot.  The whole
+// state lives in registers across all substeps of a launch; lanes talk through warp shuffles only, shared
+// memory holds what needs indexed access (gripper poses, primitive parameters, self-contact scratch).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "rod_ops.cuh"
+
+namespace dlo {
+
+typedef V3<float> f3;
+enum { KIN_FREE = 0, KIN_PINNED = 1, KIN_GRASP0 = 2 };   // kin code >= 2: grasped, slot = code - 2 = g*M + k
+enum { MAT_M = 0, MAT_L0, MAT_STRETCH, MAT_ALPHA, MAT_GAMMA, MAT_SIGY, MAT_RC, MAT_MUR, MAT_MUS, MAT_N };
+enum { ROW_X = 0, ROW_V = 3, ROW_D1 = 6, ROW_KB = 9, STATE_ROWS = 11 };
+enum { FLAG_NONFINITE = 1, FLAG_CAND_OVERFLOW = 2 };
+#define DLO_FULL 0xffffffffu
+enum { PRIM_NP = 10, PRIM_SM_STRIDE = 16 };   // boxes are expanded to centre(3), half(3), R(9) in shared memory
+
+struct KParams {
+  int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
+  int G, M, K, cand_cap;
+  float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
+  int prim_type[16];
+  const float* mat;      // [B][MAT_N]
+  const uint8_t* kin;    // [B][NS]
+  const float* qloc;     // [B][G*M][3]
+  const float* pose0;    // [B][G][6]
+  const float* finger;   // [B][G][4]
+  const float* prim;     // [B][K][10]
+  const float* actions;  // [H][B][G][6]
+  float* state;          // [B][11][NS]
+  float* ckpt;           // [n_ckpt][B][11][NS]
+  float* tape;           // [stride*n_sub][B][11][NS]
+  int* flags;            // [B]
+  // per-warp shared memory layout (float offsets from the warp's base), set by the host
+  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_warp_floats;
+};
+
+// per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
+enum { POSE_P0 = 0, POSE_R0 = 3, POSE_P1 = 12, POSE_R1 = 15, POSE_FA0 = 24, POSE_FB0 = 27, POSE_FA1 = 30, POSE_FB1 = 33, POSE_RF = 36, POSE_STRIDE = 40 };
+
+__device__ __forceinline__ float shfl(float v, int src) { return __shfl_sync(DLO_FULL, v, src); }
+__device__ __forceinline__ f3 shfl3(const f3& v, int src) { return mk3<float>(shfl(v.x, src), shfl(v.y, src), shfl(v.z, src)); }
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(DLO_FULL, v, o);
+  return v;
+}
+__device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
+__device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
+
+template <int VPL> struct Topo {
+  int lane, base, nv, ks, nl, pl;   // own lane, first vertex, #valid vertices, last valid slot, next / previous lane
+  bool vvalid[VPL], evalid[VPL], interior[VPL], remote_edge;   // remote_edge: the edge at slot ks crosses to lane nl
+  __device__ __forceinline__ void init(const KParams& P) {
+    lane = threadIdx.x & 31;
+    base = lane * VPL;
+    nv = min(max(P.N - base, 0), VPL);
+    ks = nv - 1;
+    const int last_lane = (P.N - 1) / VPL;
+    nl = (base + VPL < P.N) ? lane + 1 : 0;
+    pl = (lane > 0) ? lane - 1 : last_lane;
+    if (lane > last_lane) { nl = lane; pl = lane; }
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const int i = base + k;
+      vvalid[k] = i < P.N;
+      evalid[k] = i < P.E;
+      interior[k] = vvalid[k] && (P.ring || (i >= 1 && i <= P.N - 2));
+    }
+    remote_edge = nv > 0 && (base + ks) < P.E && (base + ks + 1 >= P.N || ks == VPL - 1);
+  }
+};
+
+// one row of a state block: NS is a multiple of 4, base = lane*VPL is even
+template <int VPL> __device__ __forceinline__ void load_row(const float* __restrict__ row, int base, int NS, float out[VPL]) {
+  if (VPL % 4 == 0) {
+#pragma unroll
+    for (int k = 0; k < VPL; k += 4) {
+      float4 q = (base + k < NS) ? *reinterpret_cast<const float4*>(row + base + k) : make_float4(0.f, 0.f, 0.f, 0.f);
+      out[k] = q.x; out[k + 1] = q.y; out[k + 2] = q.z; out[k + 3] = q.w;
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < VPL; k += 2) {
+      float2 q = (base + k < NS) ? *reinterpret_cast<const float2*>(row + base + k) : make_float2(0.f, 0.f);
+      out[k] = q.x; out[k + 1] = q.y;
+    }
+  }
+}
+template <int VPL> __device__ __forceinline__ void store_row(float* __restrict__ row, int base, int NS, const float in[VPL]) {
+  if (VPL % 4 == 0) {
+#pragma unroll
+    for (int k = 0; k < VPL; k += 4)
+      if (base + k < NS) *reinterpret_cast<float4*>(row + base + k) = make_float4(in[k], in[k + 1], in[k + 2], in[k + 3]);
+  } else {
+#pragma unroll
+    for (int k = 0; k < VPL; k += 2)
+      if (base + k < NS) *reinterpret_cast<float2*>(row + base + k) = make_float2(in[k], in[k + 1]);
+  }
+}
+
+// the per-lane slice of one env's state (x, v per vertex; d1 per edge; rest curvature per vertex)
+template <int VPL> struct LaneState {
+  f3 x[VPL], v[VPL], d1[VPL];
+  float kb1[VPL], kb2[VPL];
+};
+
+template <int VPL> __device__ __forceinline__ void load_state(const float* __restrict__ blk, int base, int NS, LaneState<VPL>& s) {
+  float r[STATE_ROWS][VPL];
+#pragma unroll
+  for (int q = 0; q < STATE_ROWS; ++q) load_row<VPL>(blk + q * NS, base, NS, r[q]);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    s.x[k] = mk3<float>(r[0][k], r[1][k], r[2][k]);
+    s.v[k] = mk3<float>(r[3][k], r[4][k], r[5][k]);
+    s.d1[k] = mk3<float>(r[6][k], r[7][k], r[8][k]);
+    s.kb1[k] = r[9][k]; s.kb2[k] = r[10][k];
+  }
+}
+template <int VPL> __device__ __forceinline__ void store_state(float* __restrict__ blk, int base, int NS, const LaneState<VPL>& s) {
+  float r[VPL];
+#define DLO_ST(q, expr) { _Pragma("unroll") for (int k = 0; k < VPL; ++k) r[k] = (expr); store_row<VPL>(blk + (q) * NS, base, NS, r); }
+  DLO_ST(0, s.x[k].x) DLO_ST(1, s.x[k].y) DLO_ST(2, s.x[k].z)
+  DLO_ST(3, s.v[k].x) DLO_ST(4, s.v[k].y) DLO_ST(5, s.v[k].z)
+  DLO_ST(6, s.d1[k].x) DLO_ST(7, s.d1[k].y) DLO_ST(8, s.d1[k].z)
+  DLO_ST(9, s.kb1[k]) DLO_ST(10, s.kb2[k])
+#undef DLO_ST
+}
+
+// per-env constants held in registers for the whole launch
+template <int VPL> struct EnvConst {
+  float m, inv_m, l0, stretch, alpha, gamma, sigy, rc, mu_r, mu_s;
+  float w[VPL];       // inverse mass, 0 for pinned / grasped / padding
+  int kin[VPL];
+  float wr;           // inverse mass of the remote next vertex (slot 0 of lane nl)
+};
+
+template <int VPL> __device__ __forceinline__ void load_env(const KParams& P, int env, const Topo<VPL>& tp, EnvConst<VPL>& c) {
+  const float* M = P.mat + (size_t)env * MAT_N;
+  c.m = M[MAT_M]; c.inv_m = 1.0f / c.m; c.l0 = M[MAT_L0]; c.stretch = M[MAT_STRETCH]; c.alpha = M[MAT_ALPHA];
+  c.gamma = M[MAT_GAMMA]; c.sigy = M[MAT_SIGY]; c.rc = M[MAT_RC]; c.mu_r = M[MAT_MUR]; c.mu_s = M[MAT_MUS];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    c.kin[k] = tp.vvalid[k] ? (int)P.kin[(size_t)env * P.NS + tp.base + k] : KIN_PINNED;
+    c.w[k] = (tp.vvalid[k] && c.kin[k] == KIN_FREE) ? c.inv_m : 0.0f;
+  }
+  c.wr = shfl(c.w[0], tp.nl);
+}
+
+// cached edge geometry of the CURRENT positions: unit tangent and inverse length per owned edge, plus the copy
+// of the previous lane's last edge (tangent, inverse length, director) needed by the bending element at slot 0
+template <int VPL> struct EdgeCache {
+  f3 t[VPL];
+  float iL[VPL];
+  f3 pt, pd1;
+  float piL;
+};
+
+template <int VPL> __device__ __forceinline__ f3 pick_last(const f3 a[VPL], int ks) {
+  f3 r = a[0];
+#pragma unroll
+  for (int k = 1; k < VPL; ++k) if (k == ks) r = a[k];
+  return r;
+}
+template <int VPL> __device__ __forceinline__ float pick_last(const float a[VPL], int ks) {
+  float r = a[0];
+#pragma unroll
+  for (int k = 1; k < VPL; ++k) if (k == ks) r = a[k];
+  return r;
+}
+
+// next-vertex value of slot k: local slot k+1, or the remote value at the lane's last slot
+template <int VPL> __device__ __forceinline__ f3 next_of(const f3 a[VPL], const f3& remote, int k, int ks) {
+  if (k == VPL - 1) return remote;
+  return (k == ks) ? remote : a[k + 1 < VPL ? k + 1 : k];
+}
+
+template <int VPL> __device__ __forceinline__ void edge_refresh(const Topo<VPL>& tp, const LaneState<VPL>& s, EdgeCache<VPL>& ec) {
+  const f3 xr = shfl3(s.x[0], tp.nl);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    f3 e = next_of<VPL>(s.x, xr, k, tp.ks) - s.x[k];
+    float L2 = dot(e, e);
+    float iL = tp.evalid[k] ? rsqrt_(L2) : 0.0f;
+    ec.iL[k] = iL;
+    ec.t[k] = iL * e;
+  }
+}
+template <int VPL> __device__ __forceinline__ void edge_prev_refresh(const Topo<VPL>& tp, const LaneState<VPL>& s, EdgeCache<VPL>& ec) {
+  ec.pt = shfl3(pick_last<VPL>(ec.t, tp.ks), tp.pl);
+  ec.pd1 = shfl3(pick_last<VPL>(s.d1, tp.ks), tp.pl);
+  ec.piL = shfl(pick_last<VPL>(ec.iL, tp.ks), tp.pl);
+}
+
+}  // namespace dlo

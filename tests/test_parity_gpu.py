@@ -1,0 +1,92 @@
+"""-m gpu: the CUDA path (through the C-ABI) against the fp64 oracle on the same seeded inputs, element by element.
+
+Forward parity: max vertex distance / rope length <= 1e-4 after the stated horizon (BASELINE.json north_star).
+Sizes are the five configs reduced in batch (envs are independent, so a subset is sound) plus ragged vertex
+counts that exercise every lanes-per-env layout (VPL 2/4/6/8), partial last lanes, odd rings and both stretch modes.
+"""
+import numpy as np
+import pytest
+
+from parity import POS_TOL, make_problem, position_error, summarize
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def dlo():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2606_04206_b200 as pkg
+    pkg.lib()
+    return pkg
+
+
+def run_both(dlo, orc, P, horizon=None, stride=0):
+    H = P["horizon"] if horizon is None else horizon
+    sim = dlo.DloSim(P)
+    sim.rollout(H, stride)
+    got = sim.state()
+    assert sim.n_bad() == 0
+    sim.close()
+    o = orc.OracleSim(P)
+    ref = o.rollout(H, stride)
+    o.close()
+    return got, ref
+
+
+FORWARD_CASES = [
+    ("cfg1 full", dict(cfg_id=1), None),
+    ("cfg2 64 envs", dict(cfg_id=2, batch=64), None),
+    ("cfg3 64 envs", dict(cfg_id=3, batch=64), None),
+    ("cfg4 32 envs", dict(cfg_id=4, batch=32), None),
+    ("cfg5 16 envs, 300 steps", dict(cfg_id=5, batch=16, horizon=300), None),
+    ("cfg2 N=37 (VPL 2, ragged)", dict(cfg_id=2, batch=8, n_verts=37, horizon=100), None),
+    ("cfg5 N=100 (VPL 4, ragged)", dict(cfg_id=5, batch=8, n_verts=100, horizon=100), None),
+    ("cfg5 N=130 (VPL 6)", dict(cfg_id=5, batch=4, n_verts=130, horizon=60), None),
+    ("cfg5 N=200 (VPL 8)", dict(cfg_id=5, batch=4, n_verts=200, horizon=40), None),
+    ("cfg4 N=45 (odd ring)", dict(cfg_id=4, batch=8, n_verts=45, horizon=150), None),
+    ("cfg4 N=98 (even ring, ragged)", dict(cfg_id=4, batch=4, n_verts=98, horizon=100), None),
+    ("cfg1 stretch energy", dict(cfg_id=1, n_verts=24), dict(stretch_mode=0, stretch=2.0e2)),
+]
+
+
+@pytest.mark.parametrize("name,kw,over", FORWARD_CASES, ids=[c[0] for c in FORWARD_CASES])
+def test_forward_parity(dlo, orc, name, kw, over):
+    P = make_problem(**kw)
+    if over:
+        P["config"]["stretch_mode"] = over["stretch_mode"]
+        P["material"]["stretch"][:] = over["stretch"]
+    got, ref = run_both(dlo, orc, P)
+    err = position_error(P, got["x"], ref["x"])
+    print(summarize(name, err))
+    assert np.isfinite(got["x"]).all()
+    assert err.max() <= POS_TOL, summarize(name, err)
+    # frames stay unit and orthogonal to their edges (state invariant of A9)
+    E = P["config"]["n_verts"] - (0 if P["config"]["topology"] else 1)
+    d1 = got["d1"][:, :, :E]
+    assert np.abs(np.linalg.norm(d1, axis=1) - 1).max() < 1e-5
+    dref = ref["d1"][:, :, :E]
+    assert np.abs(d1 - dref).max() < 5e-3
+    assert np.abs(got["kappa_bar"] - ref["kappa_bar"]).max() < 5e-3 * max(1.0, np.abs(ref["kappa_bar"]).max())
+
+
+def test_rollout_is_repeatable_bitwise(dlo):
+    """two rollouts from the same state give identical bits (deterministic reductions, no atomics on the path)"""
+    P = make_problem(4, batch=16, horizon=120)
+    sim = dlo.DloSim(P)
+    a = sim.rollout(120, 0).state()
+    b = sim.rollout(120, 40).state()
+    sim.close()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_empty_horizon_and_call_order(dlo):
+    P = make_problem(1)
+    sim = dlo.DloSim(P)
+    s0 = sim.rollout(0, 0).state()
+    assert np.allclose(s0["x"], P["x0"], atol=1e-7)
+    with pytest.raises(dlo.DloError) as e:
+        sim.backward(np.zeros((1, 3, 32)))
+    assert e.value.status == -2
+    sim.close()
