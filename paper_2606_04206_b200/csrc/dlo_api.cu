@@ -32,7 +32,7 @@ struct dlo_sim {
   size_t blk;                     // floats per env state block
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
-  float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr;
+  float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
   uint8_t *kin = nullptr, *pins = nullptr;
   int *grasp = nullptr, *flags = nullptr;
   size_t ckpt_blocks = 0, tape_blocks = 0;
@@ -58,13 +58,14 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
   P.sm_prim = take(P.K * PRIM_SM_STRIDE);
   P.sm_q = take(P.G * P.M * 3);
   P.sm_ys = P.sm_acc = P.sm_vs = P.sm_mid = P.sm_dp = P.sm_cand = 0;
-  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = 0;
+  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = 0;
   if (P.self_contact) {
     P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
     P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap / 2);
   }
   if (adjoint) {
     P.sm_lam = take((P.N_C * VPL + P.N_C) * 32);
+    P.sm_posebar = take(P.G * 24);
     if (P.self_contact) { P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP); }
   }
   P.sm_warp_floats = o;
@@ -185,7 +186,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
 dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
   cudaStreamSynchronize(s->stream);
-  void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj,
+  void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
                  s->kin, s->pins, s->grasp, s->flags};
   for (void* p : dev) if (p) cudaFree(p);
   void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hseed_x, s->hseed_v, s->hg_act, s->hg_x0, s->hg_v0, s->hg_mat, s->hxT, s->hvT};

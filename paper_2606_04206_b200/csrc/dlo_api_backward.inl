@@ -1,12 +1,76 @@
 // dlo_api_backward.inl — dlo_backward and the host-buffer convenience calls (included by dlo_api.cu)
 
+template <int VPL> static cudaError_t launch_adjoint_t(dlo_sim* s, const KParams& P, int t0, int t1) {
+  cudaError_t e = cudaFuncSetAttribute(k_adjoint<VPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_adj > 48 * 1024 ? s->smem_adj : 48 * 1024);
+  if (e != cudaSuccess) return e;
+  const int grid = (P.B + DLO_WARPS_PER_BLOCK - 1) / DLO_WARPS_PER_BLOCK;
+  k_adjoint<VPL><<<grid, DLO_WARPS_PER_BLOCK * 32, s->smem_adj, s->stream>>>(P, t0, t1);
+  s->launches += 1;
+  return cudaGetLastError();
+}
+static cudaError_t launch_adjoint(dlo_sim* s, const KParams& P, int t0, int t1) {
+  switch (s->VPL) {
+    case 2: return launch_adjoint_t<2>(s, P, t0, t1);
+    case 4: return launch_adjoint_t<4>(s, P, t0, t1);
+    case 6: return launch_adjoint_t<6>(s, P, t0, t1);
+    default: return launch_adjoint_t<8>(s, P, t0, t1);
+  }
+}
+
 extern "C" {
 
 dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g_actions, float* g_x0, float* g_v0, float* g_material) {
   if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
   if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
-  (void)gxT; (void)gvT; (void)g_actions; (void)g_x0; (void)g_v0; (void)g_material;
-  return fail(DLO_ERR_UNSUPPORTED, "adjoint kernel not built yet");
+  const int H = s->H_done, stride = s->stride, B = s->P.B;
+  const size_t blk = s->blk, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub;
+  if (seg > s->tape_blocks) {
+    CU(cudaStreamSynchronize(s->stream));
+    if (s->tape) cudaFree(s->tape);
+    s->tape = nullptr; s->tape_blocks = 0;
+    CU(dalloc(&s->tape, seg * B * blk));
+    s->tape_blocks = seg;
+  }
+  if (!s->adj) {
+    CU(dalloc(&s->adj, (size_t)B * blk));
+    CU(dalloc(&s->replay, (size_t)B * blk));
+    CU(dalloc(&s->gmat, (size_t)B * 5));
+    if (s->P.self_contact) CU(dalloc(&s->acc_tape, (size_t)B * s->P.N_C * 3 * 32 * s->VPL));
+  }
+  const size_t nadj = (size_t)B * blk;
+  k_seed_adjoint<<<(unsigned)((nadj + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, gxT, gvT, s->adj);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  CU(cudaMemsetAsync(s->gmat, 0, (size_t)B * 5 * sizeof(float), s->stream));
+  if (g_actions && s->P.G > 0) CU(cudaMemsetAsync(g_actions, 0, (size_t)H * B * s->P.G * 6 * sizeof(float), s->stream));
+  const int nseg = (H + stride - 1) / stride;
+  for (int g = nseg - 1; g >= 0; --g) {
+    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H;
+    CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+    // replay the segment from its checkpoint, leaving the state at the start of every substep on the tape
+    KParams Pf = s->P;
+    smem_layout(Pf, s->VPL, false);
+    Pf.state = s->replay; Pf.tape = s->tape;
+    {
+      dlo_sim tmp = *s;   // launch through the same path as the forward, on the replay buffer
+      tmp.P = Pf;
+      cudaError_t e = launch_forward(&tmp, t0, t1, 0, 1);
+      s->launches = tmp.launches;
+      if (e != cudaSuccess) return fail(DLO_ERR_CUDA, std::string("replay launch: ") + cudaGetErrorString(e));
+    }
+    KParams Pa = s->P;
+    smem_layout(Pa, s->VPL, true);
+    Pa.tape = s->tape; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
+    CU(launch_adjoint(s, Pa, t0, t1));
+  }
+  if (g_x0 || g_v0) {
+    const size_t n = (size_t)B * STATE_ROWS * s->P.N;
+    k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, s->adj, g_x0, g_v0, nullptr, nullptr);
+    s->launches += 1;
+    CU(cudaGetLastError());
+  }
+  if (g_material) CU(cudaMemcpyAsync(g_material, s->gmat, (size_t)B * 5 * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  return DLO_OK;
 }
 
 static dlo_status stage(float** pinned, size_t n) {

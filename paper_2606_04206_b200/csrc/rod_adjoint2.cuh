@@ -1,0 +1,366 @@
+// rod_adjoint2.cuh — reverse of one substep (A9 ... A1) and the segment adjoint kernel (second half of rod_adjoint.cuh)
+#pragma once
+
+namespace dlo {
+
+// undo + differentiate one Eq.10 edge update.  dxk/dxn: corrections of the edge's own / next vertex AFTER the
+// update (restored to their values before it); gk/gn: their adjoints (updated in place); epb: adjoint of the
+// predicted edge vector.
+__device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float wk, float wn, float atil, f3& dxk, f3& dxn, float& S,
+                                             f3& gk, f3& gn, float& Sb, float& atilbar, f3& epb) {
+  const f3 ep = epred + (dxn - dxk);                // = (L - lam (wk+wn)) t
+  const float iLp = rsqrt_(dot(ep, ep));
+  const f3 t = iLp * ep;
+  const float L = 1.0f / iLp + lam * (wk + wn);
+  const float Spost = S;
+  S -= lam;
+  dxk = axpy(dxk, -lam * wk, t);
+  dxn = axpy(dxn, lam * wn, t);
+  f3 eb;
+  project_edge_adj<float>(t, 1.0f / L, lam, Spost, wk, wn, atil, gk, gn, Sb, atilbar, eb);
+  gn += eb;
+  gk -= eb;
+  epb += eb;
+}
+
+// Reverse of one substep.  s0 = state at its start (from the tape); A: in = adjoint of the state at its end,
+// out = adjoint of the state at its start.  G accumulates material / action adjoints of this lane.
+template <int VPL>
+__device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
+                                                const float ap[6], const float ac[6], int sub, const LaneState<VPL>& s0,
+                                                LaneAdj<VPL>& A, GradAcc& G, float* acc_tape) {
+  const float h = P.h, inv_h = P.inv_h;
+  // ---- forward recompute with recording
+  LaneState<VPL> s = s0;
+  EdgeCache<VPL> ec0, ec;
+  edge_refresh<VPL>(tp, s0, ec0);
+  edge_prev_refresh<VPL>(tp, s0, ec0);
+  ec = ec0;
+  SubRec<VPL> R;
+  if (P.G > 0) {
+    for (int k = tp.lane; k < P.G * 24; k += 32) sm.posebar[k] = 0.0f;
+  }
+  substep<VPL, true>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape);
+  if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
+
+  f3 tbar_old[VPL], tbar_new[VPL];
+  float iLbar_old[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) { tbar_old[k] = zero3<float>(); tbar_new[k] = zero3<float>(); iLbar_old[k] = 0.0f; }
+
+  // ---- reverse A9: plasticity (Eq.11), then the frame transport
+  if (P.plasticity) {
+    const float Y = c.sigy * c.l0;
+    f3 ptb = zero3<float>(), pdb = zero3<float>();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      if (tp.interior[k]) {
+        const f3 ta = (k == 0) ? ec.pt : ec.t[k > 0 ? k - 1 : 0];
+        const f3 da = (k == 0) ? ec.pd1 : s.d1[k > 0 ? k - 1 : 0];
+        float k1, k2;
+        material_curvature<float>(ta, ec.t[k], da, s.d1[k], k1, k2);
+        float k1bar = 0.f, k2bar = 0.f, Ybar = 0.f;
+        plasticity_adj<float>(k1, k2, s0.kb1[k], s0.kb2[k], Y, c.rc, A.kb1[k], A.kb2[k], k1bar, k2bar, Ybar, G.gm[GM_RC]);
+        G.gm[GM_SIGY] += Ybar * c.l0;
+        f3 tab = zero3<float>(), tbb = zero3<float>(), dab = zero3<float>(), dbb = zero3<float>();
+        material_curvature_adj<float>(ta, ec.t[k], da, s.d1[k], k1bar, k2bar, tab, tbb, dab, dbb);
+        tbar_new[k] += tbb;
+        A.d1[k] += dbb;
+        if (k == 0) { ptb += tab; pdb += dab; }
+        else { tbar_new[k > 0 ? k - 1 : 0] += tab; A.d1[k > 0 ? k - 1 : 0] += dab; }
+      }
+    }
+    add_at_last<VPL>(tbar_new, tp.ks, shfl3(ptb, tp.nl));
+    add_at_last<VPL>(A.d1, tp.ks, shfl3(pdb, tp.nl));
+  }
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    if (tp.evalid[k]) {
+      f3 tob = zero3<float>(), tnb = zero3<float>(), dob = zero3<float>();
+      frame_update_adj<float>(R.t_old[k], ec.t[k], s0.d1[k], A.d1[k], tob, tnb, dob);
+      tbar_old[k] += tob; tbar_new[k] += tnb; A.d1[k] = dob;
+    } else A.d1[k] = zero3<float>();
+  }
+  {   // new tangents -> new positions
+    f3 send = zero3<float>();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.evalid[k]) scatter_edge<VPL>(A.x, send, k, tp.ks, normalize_adj<float>(ec.t[k], ec.iL[k], tbar_new[k], 0.0f));
+    A.x[0] += shfl3(send, tp.pl);
+  }
+
+  // ---- reverse A8 commit
+  f3 velbar[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    velbar[k] = zero3<float>();
+    if (c.kin[k] == KIN_FREE) velbar[k] = axpy(A.v[k], h, A.x[k]);
+    else if (c.kin[k] >= KIN_GRASP0) { grasp_target_adj(P, sm, c.kin[k], A.x[k]); velbar[k] = A.v[k]; A.x[k] = zero3<float>(); }
+    A.v[k] = zero3<float>();
+  }
+
+  // ---- reverse A7 rigid coupling
+  f3 ybar[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    ybar[k] = zero3<float>();
+    if (c.kin[k] == KIN_FREE && R.active[k]) rigid_coupling_adj(P, sm, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k], ybar[k]);
+  }
+
+  // ---- reverse A6 friction + reconciliation.  velbar is now the adjoint of v^3.
+  if (P.self_contact && R.ncand > 0) {
+    for (int p = tp.lane; p < R.ncand; p += 32) sm.dpbar[p] = 0.0f;
+    __syncwarp();
+  }
+  if (P.self_contact && R.any_pen) {
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const int i = tp.base + k;
+      sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
+      sts3(sm.vs, sm.NP, i, (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k]);
+      sts3(sm.vbar, sm.NP, i, (c.kin[k] == KIN_FREE) ? velbar[k] : zero3<float>());
+      sts3(sm.ybar, sm.NP, i, zero3<float>());
+    }
+    __syncwarp();
+    friction_pass_adj<VPL>(P, tp, sm, R.ncand, c.mu_s);
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const int i = tp.base + k;
+      velbar[k] += lds3(sm.acc, sm.NP, i);
+      ybar[k] += lds3(sm.ybar, sm.NP, i);
+      sts3(sm.acc, sm.NP, i, zero3<float>());
+    }
+    __syncwarp();
+  }
+  f3 v1bar[VPL], dxb[VPL], xpb[VPL], epb[VPL];
+  float Sb[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    v1bar[k] = velbar[k];
+    dxb[k] = (c.kin[k] == KIN_FREE) ? axpy(ybar[k], inv_h, velbar[k]) : ybar[k];
+    xpb[k] = ybar[k];
+    epb[k] = zero3<float>();
+    Sb[k] = 0.0f;
+  }
+
+  // ---- reverse A5: iterations backwards; each Eq.10 update is undone from its stored multiplier
+  const f3 xpr = shfl3(R.xp[0], tp.nl);
+  f3 epred[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
+  const float atil = c.stretch * inv_h * inv_h;
+  float atilbar = 0.0f;
+  for (int it = P.N_C - 1; it >= 0; --it) {
+    if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) {
+        const int i = tp.base + k;
+        R.dx[k] -= lds3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i);
+        sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
+        sts3(sm.vbar, sm.NP, i, dxb[k]);
+        sts3(sm.ybar, sm.NP, i, zero3<float>());
+      }
+      __syncwarp();
+      contact_pass_adj<VPL>(P, tp, sm, R.ncand);
+      __syncwarp();
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) {
+        const f3 yb = lds3(sm.ybar, sm.NP, tp.base + k);
+        dxb[k] += yb;
+        xpb[k] += yb;
+      }
+      __syncwarp();
+    }
+    if (P.stretch_mode == 1) {
+      if (P.odd_ring) {   // third colour
+        f3 dxr = shfl3(R.dx[0], tp.nl), gr = shfl3(dxb[0], tp.nl);
+        const f3 dxr0 = dxr, gr0 = gr;
+#pragma unroll
+        for (int k = 0; k < VPL; k += 2) {
+          if (k == tp.ks && tp.base + k == P.E - 1 && c.w[k] + c.wr > 0.0f)
+            edge_reverse(epred[k], sm.lam[(P.N_C * VPL + it) * 32 + tp.lane], c.w[k], c.wr, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
+        }
+        R.dx[0] += shfl3(dxr - dxr0, tp.pl);
+        dxb[0] += shfl3(gr - gr0, tp.pl);
+      }
+      {   // black
+        f3 dxr = shfl3(R.dx[0], tp.nl), gr = shfl3(dxb[0], tp.nl);
+        const f3 dxr0 = dxr, gr0 = gr;
+#pragma unroll
+        for (int k = 1; k < VPL; k += 2) {
+          const bool rem = (k == VPL - 1) || (k == tp.ks);
+          const bool on = tp.evalid[k] && (k <= tp.ks);
+          const float wn = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
+          if (on && c.w[k] + wn > 0.0f) {
+            const float lam = sm.lam[(it * VPL + k) * 32 + tp.lane];
+            if (rem) edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
+            else edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], R.dx[k + 1 < VPL ? k + 1 : k], R.S[k], dxb[k], dxb[k + 1 < VPL ? k + 1 : k], Sb[k], atilbar, epb[k]);
+          }
+        }
+        R.dx[0] += shfl3(dxr - dxr0, tp.pl);
+        dxb[0] += shfl3(gr - gr0, tp.pl);
+      }
+#pragma unroll
+      for (int k = 0; k < VPL; k += 2) {   // red
+        const bool on = (k + 1 < tp.nv) && tp.evalid[k];
+        if (on && c.w[k] + c.w[k + 1] > 0.0f)
+          edge_reverse(epred[k], sm.lam[(it * VPL + k) * 32 + tp.lane], c.w[k], c.w[k + 1], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
+      }
+    }
+  }
+  G.gm[GM_STRETCH] += (P.stretch_mode == 1) ? atilbar * inv_h * inv_h : 0.0f;
+  {   // predicted edge vectors -> predicted positions
+    f3 send = zero3<float>();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.evalid[k]) scatter_edge<VPL>(xpb, send, k, tp.ks, epb[k]);
+    xpb[0] += shfl3(send, tp.pl);
+  }
+
+  // ---- reverse A4 predict, A3 velocity
+  const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
+  f3 fbar[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    v1bar[k] = axpy(v1bar[k], h, xpb[k]);
+    if (tp.vvalid[k]) A.x[k] += xpb[k];
+    fbar[k] = zero3<float>();
+    if (c.kin[k] == KIN_FREE) {
+      A.v[k] = idamp * v1bar[k];
+      fbar[k] = (hm * idamp) * v1bar[k];
+      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], R.v1[k]);
+    } else if (c.kin[k] >= KIN_GRASP0) {
+      const f3 tb = inv_h * v1bar[k];
+      grasp_target_adj(P, sm, c.kin[k], tb);
+      A.x[k] -= tb;
+    }
+  }
+
+  // ---- reverse A2 forces: bending elements (and the stretch force in ENERGY mode) -> old edge geometry
+  {
+    const f3 fb_prev = shfl3(pick_last<VPL>(fbar, tp.ks), tp.pl), fb_next = shfl3(fbar[0], tp.nl);
+    const float sc = c.alpha / c.l0;
+    f3 ptb = zero3<float>(), pdb = zero3<float>();
+    float piLb = 0.0f, sbar = 0.0f;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      if (tp.interior[k]) {
+        const f3 ta = (k == 0) ? ec0.pt : ec0.t[k > 0 ? k - 1 : 0];
+        const f3 da = (k == 0) ? ec0.pd1 : s0.d1[k > 0 ? k - 1 : 0];
+        const float ia = (k == 0) ? ec0.piL : ec0.iL[k > 0 ? k - 1 : 0];
+        const f3 Gab = ((k == 0) ? fb_prev : fbar[k > 0 ? k - 1 : 0]) - fbar[k];
+        const f3 Gbb = fbar[k] - next_of<VPL>(fbar, fb_next, k, tp.ks);
+        f3 tab = zero3<float>(), tbb = zero3<float>(), dab = zero3<float>(), dbb = zero3<float>();
+        float iab = 0.f, ibb = 0.f;
+        bend_element_adj<float>(ta, ec0.t[k], ia, ec0.iL[k], da, s0.d1[k], s0.kb1[k], s0.kb2[k], sc, Gab, Gbb, tab, tbb, iab, ibb, dab, dbb,
+                                A.kb1[k], A.kb2[k], sbar);
+        tbar_old[k] += tbb; iLbar_old[k] += ibb; A.d1[k] += dbb;
+        if (k == 0) { ptb += tab; pdb += dab; piLb += iab; }
+        else { tbar_old[k > 0 ? k - 1 : 0] += tab; A.d1[k > 0 ? k - 1 : 0] += dab; iLbar_old[k > 0 ? k - 1 : 0] += iab; }
+      }
+    }
+    G.gm[GM_ALPHA] += sbar / c.l0;
+    add_at_last<VPL>(tbar_old, tp.ks, shfl3(ptb, tp.nl));
+    add_at_last<VPL>(A.d1, tp.ks, shfl3(pdb, tp.nl));
+    add_at_last<VPL>(iLbar_old, tp.ks, shfl(piLb, tp.nl));
+    if (P.stretch_mode == 0) {
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) {
+        if (tp.evalid[k]) {
+          const f3 Fb = fbar[k] - next_of<VPL>(fbar, fb_next, k, tp.ks);
+          const float L = 1.0f / ec0.iL[k], eps = L / c.l0 - 1.0f, Ft = dot(Fb, ec0.t[k]);
+          G.gm[GM_STRETCH] += eps * Ft;
+          tbar_old[k] += (c.stretch * eps) * Fb;
+          iLbar_old[k] -= (c.stretch * Ft / c.l0) * L * L;
+        }
+      }
+    }
+    f3 send = zero3<float>();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.evalid[k]) scatter_edge<VPL>(A.x, send, k, tp.ks, normalize_adj<float>(ec0.t[k], ec0.iL[k], tbar_old[k], iLbar_old[k]));
+    A.x[0] += shfl3(send, tp.pl);
+  }
+
+  // ---- reverse A1: pose adjoints -> action adjoints (lane g owns gripper g)
+  if (P.G > 0) {
+    __syncwarp();
+    if (tp.lane < P.G) {
+      const float tau0 = (float)sub / (float)P.n_sub, tau1 = (float)(sub + 1) / (float)P.n_sub;
+      PoseBar<float> b0, b1;
+      const float* pb = sm.posebar + tp.lane * 24;
+      b0.p = mk3<float>(pb[0], pb[1], pb[2]); b1.p = mk3<float>(pb[12], pb[13], pb[14]);
+#pragma unroll
+      for (int k = 0; k < 9; ++k) { b0.R[k] = pb[3 + k]; b1.R[k] = pb[15 + k]; }
+      make_pose_adj<float>(ap, ac, tau0, b0, G.apbar, G.acbar);
+      make_pose_adj<float>(ap, ac, tau1, b1, G.apbar, G.acbar);
+    }
+    __syncwarp();
+  }
+}
+
+// Segment adjoint: walks the substeps of steps t1-1 .. t0 backwards, one warp per env.  P.tape holds the state at
+// the start of every substep of the segment (written by k_forward), P.adj the running state adjoint.
+template <int VPL>
+__global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_adjoint(const __grid_constant__ KParams P, int t0, int t1) {
+  extern __shared__ __align__(16) float smem[];
+  const int wib = threadIdx.x >> 5, env = blockIdx.x * DLO_WARPS_PER_BLOCK + wib;
+  if (env >= P.B) return;
+  WarpSmem sm;
+  sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 32 * VPL);
+  Topo<VPL> tp;
+  tp.init(P);
+  EnvConst<VPL> c;
+  load_env<VPL>(P, env, tp, c);
+  warp_setup<VPL>(P, env, tp.lane, sm);
+  const size_t blk = (size_t)STATE_ROWS * P.NS;
+  LaneAdj<VPL> A;
+  load_adj<VPL>(P.adj + (size_t)env * blk, tp.base, P.NS, A);
+  GradAcc G;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) G.gm[k] = 0.0f;
+  float ap[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, ac[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+  float* acc_tape = P.acc_tape ? P.acc_tape + (size_t)env * P.N_C * 3 * sm.NP : nullptr;
+  for (int t = t1 - 1; t >= t0; --t) {
+    if (P.G > 0) load_actions(P, env, tp.lane, t, ap, ac);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { G.apbar[k] = 0.0f; G.acbar[k] = 0.0f; }
+    for (int sub = P.n_sub - 1; sub >= 0; --sub) {
+      LaneState<VPL> s0;
+      load_state<VPL>(P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk, tp.base, P.NS, s0);
+      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0, A, G, acc_tape);
+    }
+    if (P.g_actions && tp.lane < P.G) {
+      float* gc = P.g_actions + (((size_t)t * P.B + env) * P.G + tp.lane) * 6;
+#pragma unroll
+      for (int k = 0; k < 6; ++k) gc[k] += G.acbar[k];
+      if (t > 0) {
+        float* gp = P.g_actions + (((size_t)(t - 1) * P.B + env) * P.G + tp.lane) * 6;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) gp[k] += G.apbar[k];
+      }
+    }
+  }
+  store_adj<VPL>(P.adj + (size_t)env * blk, tp.base, P.NS, A);
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const float tot = warp_sum(G.gm[k]);
+    if (tp.lane == 0) P.gmat[(size_t)env * 5 + k] += tot;
+  }
+}
+
+// seeds of the reverse pass -> running adjoint block; gradients out of it
+__global__ void k_seed_adjoint(int B, int N, int NS, const float* gx, const float* gv, float* adj) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)B * STATE_ROWS * NS) return;
+  const int i = (int)(idx % NS), q = (int)((idx / NS) % STATE_ROWS), env = (int)(idx / ((size_t)NS * STATE_ROWS));
+  float val = 0.0f;
+  if (i < N) {
+    if (q < 3 && gx) val = gx[((size_t)env * 3 + q) * N + i];
+    else if (q >= 3 && q < 6 && gv) val = gv[((size_t)env * 3 + q - 3) * N + i];
+  }
+  adj[idx] = val;
+}
+
+}  // namespace dlo

@@ -7,13 +7,13 @@
 namespace dlo {
 
 struct WarpSmem {
-  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar;
+  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar;
   unsigned short* cand;
   int NP;   // 32*VPL
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
-    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar;
+    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar;
     NP = np;
   }
 };

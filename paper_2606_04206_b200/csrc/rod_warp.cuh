@@ -38,8 +38,12 @@ struct KParams {
   float* ckpt;           // [n_ckpt][B][11][NS]
   float* tape;           // [stride*n_sub][B][11][NS]
   int* flags;            // [B]
+  float* adj;            // [B][11][NS] running state adjoint of the reverse pass
+  float* acc_tape;       // [B][N_C][3][32*VPL] self-contact corrections of the substep being reversed
+  float* gmat;           // [B][5] running material gradient
+  float* g_actions;      // [H][B][G][6] (may be null)
   // per-warp shared memory layout (float offsets from the warp's base), set by the host
-  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_warp_floats;
+  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_warp_floats;
 };
 
 // per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
