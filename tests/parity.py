@@ -22,3 +22,25 @@ def gradient_error(g_gpu, g_orc):
 
 def summarize(name, err):
     return "%s: max %.3e  p99 %.3e  median %.3e  (n=%d)" % (name, err.max(), np.quantile(err, 0.99), np.median(err), len(err))
+
+
+def perturbed(P, rng, eps=2.0 ** -24):
+    """the same problem with every real input moved by one fp32 rounding (relative 2^-24, Gaussian)"""
+    Q = dict(P)
+    for k in ("x0", "actions", "init_pose"):
+        if P.get(k) is not None:
+            Q[k] = P[k] * (1.0 + eps * rng.standard_normal(P[k].shape))
+    Q["material"] = {k: v * (1.0 + eps * rng.standard_normal(v.shape)) for k, v in P["material"].items()}
+    return Q
+
+
+def oracle_position_spread(orc, P, H, ref_x, draws=2, seed=11):
+    """per-env response of the ORACLE's final positions to fp32-sized input perturbations (its conditioning):
+    max over `draws` perturbed fp64 runs of the position error against the unperturbed run"""
+    rng = np.random.default_rng(seed)
+    spread = 0.0
+    for _ in range(draws):
+        q = orc.OracleSim(perturbed(P, rng))
+        spread = np.maximum(spread, position_error(P, q.rollout(H, 0)["x"], ref_x))
+        q.close()
+    return spread

@@ -5,7 +5,7 @@ horizon exercise the ragged last segment."""
 import numpy as np
 import pytest
 
-from parity import GRAD_TOL, gradient_error, loss_and_seed, make_problem, summarize
+from parity import GRAD_TOL, gradient_error, loss_and_seed, make_problem, perturbed, summarize
 
 pytestmark = pytest.mark.gpu
 
@@ -47,16 +47,6 @@ def check(name, got, ref, keys, tol=GRAD_TOL):
 
 def env_first(k, a):
     return np.moveaxis(a, 1, 0) if k == "g_actions" else a
-
-
-def perturbed(P, rng, eps=2.0 ** -24):
-    """the same problem with every real input moved by one fp32 rounding (relative 2^-24, Gaussian)"""
-    Q = dict(P)
-    for k in ("x0", "actions", "init_pose"):
-        if P.get(k) is not None:
-            Q[k] = P[k] * (1.0 + eps * rng.standard_normal(P[k].shape))
-    Q["material"] = {k: v * (1.0 + eps * rng.standard_normal(v.shape)) for k, v in P["material"].items()}
-    return Q
 
 
 def apply_over(P, over):
