@@ -78,27 +78,39 @@ def oracle_leg(problem, mode, budget_s, steps=1, warmup=0):
     from oracle import dlo_oracle as orc
     cores = orc.num_threads()
     H_full, stride = problem["horizon"], problem["checkpoint_stride"]
-    envs = np.arange(0, problem["config"]["batch"], max(1, problem["config"]["batch"] // cores))[:cores]
-    # forward: `cores` envs x a horizon sized for the budget; fwd+bwd uses the tape-AD instantiation (much slower)
-    H = min(H_full, 100 if mode == "fwd" else 4)
-    times = []
-    for it in range(warmup + steps):
+    B = problem["config"]["batch"]
+
+    def one(envs, H):
         sim = orc.OracleSim(problem, envs=envs)
         t0 = time.perf_counter()
-        st = sim.rollout(H, min(stride, H) if mode != "fwd" else 0)
+        st = sim.rollout(H, max(1, min(stride, H)) if mode != "fwd" else 0)
         if mode != "fwd":
-            _, seed = loss_and_seed(dict(problem, loss=dict(problem["loss"], target=problem["loss"]["target"][envs])), st["x"])
+            sub = dict(problem, loss=dict(problem["loss"], target=problem["loss"]["target"][envs]))
+            _, seed = loss_and_seed(sub, st["x"])
             sim.backward(seed)
         dt = time.perf_counter() - t0
         sim.close()
+        return dt
+
+    envs = np.arange(min(B, cores))
+    probe_H = 4
+    rate = len(envs) * probe_H / one(envs, probe_H)          # env-steps/s, rough
+    # size the sample for ~budget_s/2 per pass: grow the horizon first, then the number of envs
+    units = max(rate * budget_s * 0.5, len(envs) * probe_H)
+    H = int(min(H_full, max(probe_H, units // len(envs))))
+    n_env = int(min(B, max(len(envs), (units // H) // cores * cores)))
+    envs = np.arange(n_env)
+    times = []
+    for it in range(warmup + steps):
+        dt = one(envs, H)
         if it >= warmup:
             times.append(dt)
         if sum(times) > budget_s:
             break
     t = float(np.mean(times))
     return {"value": len(envs) * H / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%d envs x %d steps of config 5 (%s, fp64%s), %.1f s per pass" % (
-                len(envs), H, mode, ", tape-AD reverse" if mode != "fwd" else "", t)}, t, len(envs) * H
+            "sample": "%d envs x %d steps of config %d (%s, fp64%s), %.1f s per pass" % (
+                len(envs), H, problem.get("config_id", 5), mode, ", tape-AD reverse" if mode != "fwd" else "", t)}, t, len(envs) * H
 
 
 def main():
@@ -107,7 +119,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="fwd", choices=["fwd", "fwdbwd"])
+    ap.add_argument("--mode", default="fwdbwd", choices=["fwd", "fwdbwd"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--batch", type=int, default=None, help="per-GPU batch (default: the config's)")
     ap.add_argument("--horizon", type=int, default=None)
@@ -131,8 +143,8 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        problem = make_problem(args.config, batch=min(B, 256), horizon=H)
-        cb, t, units = oracle_leg(problem, args.mode, budget_s=120, steps=args.steps, warmup=min(args.warmup, 1))
+        problem = make_problem(args.config, batch=min(B, 256), horizon=H, stride=full["stride"])
+        cb, t, units = oracle_leg(problem, args.mode, budget_s=60, steps=args.steps, warmup=min(args.warmup, 1))
         line = dict(base, impl="reference", value=cb["value"], ms_per_step=t * 1e3, dtype="f64", cpu_baseline=cb,
                     e2e={"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, gpu_launches=0)
         line["config"] = dict(line["config"], sample=cb["sample"])
@@ -253,7 +265,7 @@ def main():
                           "algorithmic_flops_per_env_step": FLOPS_PER_ENV_STEP[args.mode]},
                 envs_flagged=int(n_bad), ms_per_pass=per)
     if not args.no_cpu_baseline:
-        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H), args.mode, budget_s=30)
+        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H, stride=full["stride"]), args.mode, budget_s=20)
         line["cpu_baseline"] = cb
     print(json.dumps(line))
 
