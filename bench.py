@@ -154,6 +154,7 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2606_04206_b200 as dlo
+    from paper_2606_04206_b200.sharding import max_over_ranks
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the DLO library has no CPU path")
     if world > 1:
@@ -210,10 +211,7 @@ def main():
     launches = dlo.dlo_launch_count(sim.h) - l0
     per = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
     total_ms = ev[0].elapsed_time(ev[-1])
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)
     n_bad = sim.n_bad()
     ms_per_step = total_ms / args.steps
     value = B * H * world / (ms_per_step * 1e-3)
@@ -246,10 +244,7 @@ def main():
             e2e_pass()
         barrier()
         te = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([te], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            te = float(t.item())
+        te = max_over_ranks(te, dev)
         e2e = {"value": B * H * world / te, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
 
     if rank != 0:
