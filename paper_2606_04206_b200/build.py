@@ -7,7 +7,9 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdlo_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v",
+              # 2-ulp division / sqrt and flushed denormals: a fifth fewer instructions, far inside the 1e-4 parity budget
+              "-prec-div=false", "-prec-sqrt=false", "-ftz=true"]
 
 
 def sources():

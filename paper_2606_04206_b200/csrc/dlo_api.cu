@@ -278,10 +278,14 @@ template <int VPL> static cudaError_t launch_forward_t(dlo_sim* s, int t0, int t
 static cudaError_t launch_forward(dlo_sim* s, int t0, int t1, int stride, int write_tape) {
   smem_layout(s->P, s->VPL, false);
   switch (s->VPL) {
+#ifdef DLO_VPL_ONLY   /* development builds: one instantiation only */
+    default: return launch_forward_t<DLO_VPL_ONLY>(s, t0, t1, stride, write_tape);
+#else
     case 2: return launch_forward_t<2>(s, t0, t1, stride, write_tape);
     case 4: return launch_forward_t<4>(s, t0, t1, stride, write_tape);
     case 6: return launch_forward_t<6>(s, t0, t1, stride, write_tape);
     default: return launch_forward_t<8>(s, t0, t1, stride, write_tape);
+#endif
   }
 }
 

@@ -10,10 +10,14 @@ template <int VPL> static cudaError_t launch_adjoint_t(dlo_sim* s, const KParams
 }
 static cudaError_t launch_adjoint(dlo_sim* s, const KParams& P, int t0, int t1) {
   switch (s->VPL) {
+#ifdef DLO_VPL_ONLY   /* development builds: one instantiation only */
+    default: return launch_adjoint_t<DLO_VPL_ONLY>(s, P, t0, t1);
+#else
     case 2: return launch_adjoint_t<2>(s, P, t0, t1);
     case 4: return launch_adjoint_t<4>(s, P, t0, t1);
     case 6: return launch_adjoint_t<6>(s, P, t0, t1);
     default: return launch_adjoint_t<8>(s, P, t0, t1);
+#endif
   }
 }
 

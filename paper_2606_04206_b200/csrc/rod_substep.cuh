@@ -233,18 +233,22 @@ __device__ void friction_pass(const KParams& P, const Topo<VPL>& tp, const WarpS
   }
 }
 
-// A7 (L103): soft coupling of one free vertex at y against the K fixed primitives, then the finger capsules
-__device__ __forceinline__ unsigned rigid_coupling(const KParams& P, const WarpSmem& sm, const f3& y, f3& v, float mu_r) {
+// A7 (L103): soft coupling of one free vertex at y against the K fixed primitives, then the finger capsules.
+// Not inlined on purpose: it is called once per vertex slot and is the largest single piece of straight-line code
+// (four SDF types + fingers); one copy keeps the kernel inside the instruction cache.
+struct CoupleOut { f3 v; unsigned active; };
+__device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* __restrict__ prim_sm, const float* __restrict__ pose_sm,
+                                                 f3 y, f3 v, float mu_r) {
   unsigned active = 0u;
   for (int k = 0; k < P.K; ++k) {
     float phi;
     f3 n;
-    if (!sdf_eval_pre<float>(P.prim_type[k], sm.prim + k * PRIM_SM_STRIDE, y, phi, n)) continue;
+    if (!sdf_eval_pre<float>(P.prim_type[k], prim_sm + k * PRIM_SM_STRIDE, y, phi, n)) continue;
+    if ((P.r - phi) * P.inv_eps < P.log_thresh_lo) continue;
     if (rigid_response<float>(v, zero3<float>(), n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << k;
   }
   for (int g = 0; g < P.G; ++g) {
-    const float* o = sm.pose + g * POSE_STRIDE;
-#pragma unroll
+    const float* o = pose_sm + g * POSE_STRIDE;
     for (int fk = 0; fk < 2; ++fk) {
       const float* A = o + (fk ? POSE_FA1 : POSE_FA0);
       const float* Bp = o + (fk ? POSE_FB1 : POSE_FB0);
@@ -257,7 +261,9 @@ __device__ __forceinline__ unsigned rigid_coupling(const KParams& P, const WarpS
       if (rigid_response<float>(v, vb, n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << (P.K + 2 * g + fk);
     }
   }
-  return active;
+  CoupleOut out;
+  out.v = v; out.active = active;
+  return out;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -430,7 +436,10 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) {
     R.v3[k] = vel[k];
     R.active[k] = 0u;
-    if (c.kin[k] == KIN_FREE && (P.K > 0 || P.G > 0)) R.active[k] = rigid_coupling(P, sm, R.xp[k] + R.dx[k], vel[k], c.mu_r);
+    if (c.kin[k] == KIN_FREE && (P.K > 0 || P.G > 0)) {
+      const CoupleOut co = rigid_coupling(P, sm.prim, sm.pose, R.xp[k] + R.dx[k], vel[k], c.mu_r);
+      vel[k] = co.v; R.active[k] = co.active;
+    }
     R.v4[k] = vel[k];
   }
 
