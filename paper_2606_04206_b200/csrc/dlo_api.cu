@@ -58,10 +58,11 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
   P.sm_prim = take(P.K * PRIM_SM_STRIDE);
   P.sm_q = take(P.G * P.M * 3);
   P.sm_ys = P.sm_acc = P.sm_vs = P.sm_mid = P.sm_dp = P.sm_cand = 0;
-  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = 0;
+  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = P.sm_blk = 0;
   if (P.self_contact) {
     P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
-    P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap / 2);
+    P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap);   // candidates + prefilter survivors (ushort each)
+    P.sm_blk = take(4 * 32);
   }
   if (adjoint) {
     P.sm_lam = take((P.N_C * VPL + P.N_C) * 32);

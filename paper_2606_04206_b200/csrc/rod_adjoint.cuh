@@ -135,9 +135,11 @@ __device__ __forceinline__ void ordered_scatter_vec4(unsigned hits, int lane, fl
     __syncwarp();
   }
 }
-__device__ __forceinline__ void cand_verts(const WarpSmem& sm, int N, int p, int iv[4]) {
+template <int VPL> __device__ __forceinline__ void cand_verts(const WarpSmem& sm, int N, int p, int iv[4]) {
   const unsigned c = sm.cand[p];
   iv[0] = c >> 8; iv[2] = c & 255; iv[1] = (iv[0] + 1 < N) ? iv[0] + 1 : 0; iv[3] = (iv[2] + 1 < N) ? iv[2] + 1 : 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) iv[k] = vpos<VPL>(iv[k]);   // shared-memory positions
 }
 
 // reverse of one Eq.13 Jacobi pass: positions y (before the pass) in sm.ys, adjoint of the post-pass corrections
@@ -151,7 +153,7 @@ template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& 
     int iv[4] = {0, 0, 0, 0};
     f3 xb[4] = {zero3<float>(), zero3<float>(), zero3<float>(), zero3<float>()};
     if (p < ncand) {
-      cand_verts(sm, N, p, iv);
+      cand_verts<VPL>(sm, N, p, iv);
       f3 xs[4], ob[4];
       float ws[4];
 #pragma unroll
@@ -176,7 +178,7 @@ template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams&
     f3 xb[4] = {zero3<float>(), zero3<float>(), zero3<float>(), zero3<float>()};
     f3 vb[4] = {zero3<float>(), zero3<float>(), zero3<float>(), zero3<float>()};
     if (p < ncand && sm.dp[p] > 0.0f) {
-      cand_verts(sm, N, p, iv);
+      cand_verts<VPL>(sm, N, p, iv);
       f3 xs[4], vv[4], ob[4];
       float ws[4];
 #pragma unroll

@@ -115,7 +115,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.self_contact && R.any_pen) {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = tp.base + k;
+      const int i = k * 32 + tp.lane;
       sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
       sts3(sm.vs, sm.NP, i, (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k]);
       sts3(sm.vbar, sm.NP, i, (c.kin[k] == KIN_FREE) ? velbar[k] : zero3<float>());
@@ -126,7 +126,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = tp.base + k;
+      const int i = k * 32 + tp.lane;
       velbar[k] += lds3(sm.acc, sm.NP, i);
       ybar[k] += lds3(sm.ybar, sm.NP, i);
       sts3(sm.acc, sm.NP, i, zero3<float>());
@@ -155,7 +155,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
-        const int i = tp.base + k;
+        const int i = k * 32 + tp.lane;
         R.dx[k] -= lds3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i);
         sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
         sts3(sm.vbar, sm.NP, i, dxb[k]);
@@ -166,7 +166,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       __syncwarp();
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
-        const f3 yb = lds3(sm.ybar, sm.NP, tp.base + k);
+        const f3 yb = lds3(sm.ybar, sm.NP, k * 32 + tp.lane);
         dxb[k] += yb;
         xpb[k] += yb;
       }

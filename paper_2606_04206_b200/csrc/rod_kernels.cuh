@@ -160,7 +160,7 @@ template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  write_tape: the state at
 // the start of every substep goes to P.tape (replay half of the reverse pass).
 template <int VPL>
-__global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
+__global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32, VPL <= 4 ? 3 : 2) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
   extern __shared__ __align__(16) float smem[];
   const int wib = threadIdx.x >> 5, env = blockIdx.x * DLO_WARPS_PER_BLOCK + wib;
   if (env >= P.B) return;

@@ -7,13 +7,13 @@
 namespace dlo {
 
 struct WarpSmem {
-  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar;
+  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk;
   unsigned short* cand;
   int NP;   // 32*VPL
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
-    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar;
+    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk;
     NP = np;
   }
 };
@@ -89,9 +89,9 @@ __device__ __forceinline__ void bending_forces(const Topo<VPL>& tp, const LaneSt
   }
 }
 
-// segment-pair test used by the candidate build: exact closest distance below `lim`
-__device__ __forceinline__ bool pair_within(const float* ys, int NP, int a, int an, int b, int bn, float lim) {
-  f3 p1 = lds3(ys, NP, a), q1 = lds3(ys, NP, an), p2 = lds3(ys, NP, b), q2 = lds3(ys, NP, bn);
+// segment-pair test used by the candidate build: exact closest distance below `lim` (pa.. are smem positions)
+__device__ __forceinline__ bool pair_within(const float* ys, int NP, int pa, int pan, int pb, int pbn, float lim) {
+  f3 p1 = lds3(ys, NP, pa), q1 = lds3(ys, NP, pan), p2 = lds3(ys, NP, pb), q2 = lds3(ys, NP, pbn);
   float t, u;
   closest_points<float>(p1, q1, p2, q2, t, u);
   f3 dv = axpy(p1, t, q1 - p1) - axpy(p2, u, q2 - p2);
@@ -99,36 +99,75 @@ __device__ __forceinline__ bool pair_within(const float* ys, int NP, int a, int 
 }
 
 // A4 candidate list (Eq.13 "potentially colliding", R-15): all edge pairs a<b with cyclic index distance >=
-// self_skip closer than 2(r_a+r_b) at x^p, in lexicographic order.  ys holds x^p, mid holds (midpoint, half length).
+// self_skip whose segments are closer than 2(r_a+r_b) at x^p.  The SET equals the oracle's; it is found
+// hierarchically instead of by the all-pairs loop: (1) bounding spheres of the lanes' edge blocks (VPL edges each)
+// are tested pairwise, (2) edge pairs of the surviving block pairs pass a midpoint-sphere prefilter, (3) the
+// survivors take the exact segment-segment test, 32 at a time.  Every rejection is conservative, so no pair is
+// lost.  Order: by (block a, block b, slot a, slot b) - deterministic, but not the oracle's lexicographic order
+// (only the fp32 summation order of the Jacobi pass depends on it).  ys = x^p, mid = (midpoint, half length, w).
 template <int VPL>
-__device__ int build_candidates(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int env) {
-  const int E = P.E, N = P.N, NP = sm.NP;
+__device__ __noinline__ int build_candidates(const KParams& P, int lane, const WarpSmem& sm, int env, float bx, float by, float bz, float br) {
+  const int E = P.E, N = P.N, NP = sm.NP, nb = (E + VPL - 1) / VPL;
   const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
-  int ncand = 0;
-  for (int a = 0; a < E; ++a) {
-    const int an = (a + 1 < N) ? a + 1 : 0;
-    const float ax = sm.mid[a], ay = sm.mid[NP + a], az = sm.mid[2 * NP + a], ah = sm.mid[3 * NP + a];
-    const int bmax = P.ring ? min(E - 1, a + E - P.self_skip) : E - 1;
-    for (int b0 = a + P.self_skip; b0 <= bmax; b0 += 32) {
-      const int b = b0 + tp.lane;
-      bool hit = false;
-      if (b <= bmax) {
-        const float dx = sm.mid[b] - ax, dy = sm.mid[NP + b] - ay, dz = sm.mid[2 * NP + b] - az;
-        const float reach = ah + sm.mid[3 * NP + b] + lim;
-        if (dx * dx + dy * dy + dz * dz < reach * reach) hit = pair_within(sm.ys, NP, a, an, b, (b + 1 < N) ? b + 1 : 0, lim);
+  constexpr int PP = VPL * VPL, NPER = PP <= 32 ? 32 / PP : 1, ITER = (PP + 31) / 32;
+  unsigned short* surv = sm.cand + P.cand_cap;
+  // (1) block pairs: lane B tests its own block against block A
+  sm.blk[lane] = bx; sm.blk[32 + lane] = by; sm.blk[64 + lane] = bz; sm.blk[96 + lane] = br;
+  __syncwarp();
+  unsigned mymask = 0u;
+  for (int A = 0; A < nb; ++A) {
+    const float dx = sm.blk[A] - bx, dy = sm.blk[32 + A] - by, dz = sm.blk[64 + A] - bz, reach = sm.blk[96 + A] + br + lim;
+    const bool hit = lane >= A && lane < nb && dx * dx + dy * dy + dz * dz < reach * reach;
+    const unsigned m = __ballot_sync(DLO_FULL, hit);
+    if (lane == A) mymask = m;
+  }
+  // (2) edge pairs of surviving block pairs -> survivors of the midpoint-sphere prefilter
+  int nsurv = 0;
+  for (int A = 0; A < nb; ++A) {
+    unsigned mask = __shfl_sync(DLO_FULL, mymask, A);
+    while (mask) {
+#pragma unroll
+      for (int j = 0; j < ITER; ++j) {
+        const int sub = (PP <= 32) ? lane / PP : 0, idx = (PP <= 32) ? lane % PP : j * 32 + lane;
+        const unsigned Bsel = __fns(mask, 0, sub + 1);
+        const int ka = idx / VPL, kb = idx % VPL, a = A * VPL + ka, b = (int)Bsel * VPL + kb, d = b - a;
+        bool hit = false;
+        if (Bsel != 0xffffffffu && idx < PP && sub < NPER && b < E && d >= P.self_skip && (!P.ring || E - d >= P.self_skip)) {
+          const int pa = ka * 32 + A, pb = kb * 32 + (int)Bsel;
+          const float dx = sm.mid[pb] - sm.mid[pa], dy = sm.mid[NP + pb] - sm.mid[NP + pa], dz = sm.mid[2 * NP + pb] - sm.mid[2 * NP + pa];
+          const float reach = sm.mid[3 * NP + pa] + sm.mid[3 * NP + pb] + lim;
+          hit = dx * dx + dy * dy + dz * dz < reach * reach;
+        }
+        const unsigned m = __ballot_sync(DLO_FULL, hit);
+        if (hit) {
+          const int pos = nsurv + __popc(m & ((1u << lane) - 1u));
+          if (pos < P.cand_cap) surv[pos] = (unsigned short)((a << 8) | b);
+        }
+        nsurv += __popc(m);
       }
-      const unsigned m = __ballot_sync(DLO_FULL, hit);
-      if (hit) {
-        const int pos = ncand + __popc(m & ((1u << tp.lane) - 1u));
-        if (pos < P.cand_cap) sm.cand[pos] = (unsigned short)((a << 8) | b);
-      }
-      ncand += __popc(m);
+#pragma unroll
+      for (int q = 0; q < NPER; ++q) mask &= mask - 1u;
     }
   }
-  if (ncand > P.cand_cap) {
-    if (tp.lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
-    ncand = P.cand_cap;
+  bool overflow = nsurv > P.cand_cap;
+  nsurv = min(nsurv, P.cand_cap);
+  __syncwarp();
+  // (3) exact narrow phase on the survivors, ordered compaction into the candidate list
+  int ncand = 0;
+  for (int p0 = 0; p0 < nsurv; p0 += 32) {
+    const int p = p0 + lane;
+    bool hit = false;
+    unsigned c = 0u;
+    if (p < nsurv) {
+      c = surv[p];
+      const int a = c >> 8, b = c & 255, an = (a + 1 < N) ? a + 1 : 0, bn = (b + 1 < N) ? b + 1 : 0;
+      hit = pair_within(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn), lim);
+    }
+    const unsigned m = __ballot_sync(DLO_FULL, hit);
+    if (hit) sm.cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)c;
+    ncand += __popc(m);
   }
+  if (overflow && lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
   __syncwarp();
   return ncand;
 }
@@ -164,6 +203,8 @@ __device__ bool contact_pass(const KParams& P, const Topo<VPL>& tp, const WarpSm
     if (p < ncand) {
       const unsigned c = sm.cand[p];
       iv[0] = c >> 8; iv[2] = c & 255; iv[1] = (iv[0] + 1 < N) ? iv[0] + 1 : 0; iv[3] = (iv[2] + 1 < N) ? iv[2] + 1 : 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) iv[k] = vpos<VPL>(iv[k]);
       f3 xs[4];
       float ws[4];
 #pragma unroll
@@ -203,6 +244,8 @@ __device__ void friction_pass(const KParams& P, const Topo<VPL>& tp, const WarpS
     if (p < ncand && sm.dp[p] > 0.0f) {
       const unsigned c = sm.cand[p];
       iv[0] = c >> 8; iv[2] = c & 255; iv[1] = (iv[0] + 1 < N) ? iv[0] + 1 : 0; iv[3] = (iv[2] + 1 < N) ? iv[2] + 1 : 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) iv[k] = vpos<VPL>(iv[k]);
       f3 xs[4], vv[4];
       float ws[4];
 #pragma unroll
@@ -316,15 +359,30 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   if (P.self_contact) {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = tp.base + k;
+      const int i = k * 32 + tp.lane;   // own vertex, slot-major position
       sts3(sm.ys, sm.NP, i, R.xp[k]);
       f3 mid = axpy(R.xp[k], 0.5f, epred[k]);
       sts3(sm.mid, sm.NP, i, mid);
       sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
       sm.mid[4 * sm.NP + i] = c.w[k];
     }
+    // bounding sphere of this lane's edge block (centre = mean of its edge midpoints)
+    f3 bc = zero3<float>();
+    float bn = 0.0f, brad = -1.0e30f;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.evalid[k]) { bc += axpy(R.xp[k], 0.5f, epred[k]); bn += 1.0f; }
+    if (bn > 0.0f) {
+      bc = (1.0f / bn) * bc;
+#pragma unroll
+      for (int k = 0; k < VPL; ++k)
+        if (tp.evalid[k]) {
+          const f3 dm = axpy(R.xp[k], 0.5f, epred[k]) - bc;
+          brad = fmaxf(brad, sqrt_(dot(dm, dm)) + 0.5f * sqrt_(dot(epred[k], epred[k])));
+        }
+    }
     __syncwarp();
-    R.ncand = build_candidates<VPL>(P, tp, sm, env);
+    R.ncand = build_candidates<VPL>(P, tp.lane, sm, env, bc.x, bc.y, bc.z, brad);
     for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
     __syncwarp();
   }
@@ -392,7 +450,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     }
     if (P.self_contact && R.ncand > 0) {
 #pragma unroll
-      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, tp.base + k, R.xp[k] + R.dx[k]);
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, k * 32 + tp.lane, R.xp[k] + R.dx[k]);
       __syncwarp();
       const bool any = contact_pass<VPL>(P, tp, sm, R.ncand, c.inv_m);
       __syncwarp();
@@ -401,7 +459,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         R.jac_mask |= 1u << it;
 #pragma unroll
         for (int k = 0; k < VPL; ++k) {
-          const int i = tp.base + k;
+          const int i = k * 32 + tp.lane;   // own vertex, slot-major position
           const f3 a = lds3(sm.acc, sm.NP, i);
           R.dx[k] += a;
           if (REC) sts3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i, a);
@@ -418,13 +476,13 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) vel[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k];
   if (P.self_contact && R.any_pen) {
 #pragma unroll
-    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, tp.base + k, R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, tp.base + k, vel[k]); }
+    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, k * 32 + tp.lane, R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, k * 32 + tp.lane, vel[k]); }
     __syncwarp();
     friction_pass<VPL>(P, tp, sm, R.ncand, c.mu_s);
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = tp.base + k;
+      const int i = k * 32 + tp.lane;   // own vertex, slot-major position
       if (c.kin[k] == KIN_FREE) vel[k] += lds3(sm.acc, sm.NP, i);
       sts3(sm.acc, sm.NP, i, zero3<float>());
     }

@@ -43,7 +43,7 @@ struct KParams {
   float* gmat;           // [B][5] running material gradient
   float* g_actions;      // [H][B][G][6] (may be null)
   // per-warp shared memory layout (float offsets from the warp's base), set by the host
-  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_warp_floats;
+  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_blk, sm_warp_floats;
 };
 
 // per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
@@ -56,6 +56,9 @@ __device__ __forceinline__ float warp_sum(float v) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(DLO_FULL, v, o);
   return v;
 }
+// shared-memory position of vertex i: slot-major ((i % VPL) * 32 + i / VPL), so that the lanes' own vertices
+// (slot k of lane l -> k*32 + l) are bank-conflict free; random access by vertex index goes through vpos()
+template <int VPL> __device__ __forceinline__ int vpos(int i) { return (i % VPL) * 32 + i / VPL; }
 __device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
 __device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
 
