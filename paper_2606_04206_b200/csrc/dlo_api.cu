@@ -33,7 +33,7 @@ struct dlo_sim {
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
   float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
-  uint8_t *kin = nullptr, *pins = nullptr;
+  uint8_t *kin = nullptr, *pins = nullptr, *tape_flag = nullptr;
   int *grasp = nullptr, *flags = nullptr;
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
@@ -51,7 +51,7 @@ static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
 // per-warp shared-memory layout (float offsets); `adjoint` adds the reverse-pass scratch
 static int smem_layout(KParams& P, int VPL, bool adjoint) {
-  const int NP = 32 * VPL;
+  const int NP = 33 * VPL;   // padded row (vpos)
   int o = 0;
   auto take = [&](int n) { int at = o; o += round_up(n, 4); return at; };
   P.sm_pose = take(P.G * POSE_STRIDE);
@@ -116,7 +116,7 @@ size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
     n += ((size_t)horizon / stride + 1) * B * blk;                             // checkpoints
     n += (size_t)(stride < horizon ? stride : horizon) * P.n_sub * B * blk;    // per-substep tape of one segment
     n += B * blk;                                                              // running adjoint
-    if (P.self_contact) n += B * (size_t)P.N_C * 3 * 32 * vpl_for(P.N) * 4;    // self-contact correction tape
+    if (P.self_contact) n += B * (size_t)P.N_C * 3 * 33 * vpl_for(P.N) * 4;    // self-contact correction tape
   }
   return n;
 }
@@ -188,7 +188,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->grasp, s->flags};
+                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag};
   for (void* p : dev) if (p) cudaFree(p);
   void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hseed_x, s->hseed_v, s->hg_act, s->hg_x0, s->hg_v0, s->hg_mat, s->hxT, s->hvT};
   for (void* p : host) if (p) cudaFreeHost(p);

@@ -33,13 +33,16 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     if (s->tape) cudaFree(s->tape);
     s->tape = nullptr; s->tape_blocks = 0;
     CU(dalloc(&s->tape, seg * B * blk));
+    if (s->tape_flag) cudaFree(s->tape_flag);
+    s->tape_flag = nullptr;
+    CU(dalloc(&s->tape_flag, seg * B));
     s->tape_blocks = seg;
   }
   if (!s->adj) {
     CU(dalloc(&s->adj, (size_t)B * blk));
     CU(dalloc(&s->replay, (size_t)B * blk));
     CU(dalloc(&s->gmat, (size_t)B * 5));
-    if (s->P.self_contact) CU(dalloc(&s->acc_tape, (size_t)B * s->P.N_C * 3 * 32 * s->VPL));
+    if (s->P.self_contact) CU(dalloc(&s->acc_tape, (size_t)B * s->P.N_C * 3 * 33 * s->VPL));
   }
   const size_t nadj = (size_t)B * blk;
   k_seed_adjoint<<<(unsigned)((nadj + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, gxT, gvT, s->adj);
@@ -54,7 +57,7 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     // replay the segment from its checkpoint, leaving the state at the start of every substep on the tape
     KParams Pf = s->P;
     smem_layout(Pf, s->VPL, false);
-    Pf.state = s->replay; Pf.tape = s->tape;
+    Pf.state = s->replay; Pf.tape = s->tape; Pf.tape_flag = s->tape_flag;
     {
       dlo_sim tmp = *s;   // launch through the same path as the forward, on the replay buffer
       tmp.P = Pf;
@@ -64,7 +67,7 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     }
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
-    Pa.tape = s->tape; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
+    Pa.tape = s->tape; Pa.tape_flag = s->tape_flag; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
     CU(launch_adjoint(s, Pa, t0, t1));
   }
   if (g_x0 || g_v0) {

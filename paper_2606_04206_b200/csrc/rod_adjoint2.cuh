@@ -28,7 +28,7 @@ __device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float w
 template <int VPL>
 __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                                 const float ap[6], const float ac[6], int sub, const LaneState<VPL>& s0,
-                                                LaneAdj<VPL>& A, GradAcc& G, float* acc_tape) {
+                                                LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag) {
   const float h = P.h, inv_h = P.inv_h;
   // ---- forward recompute with recording
   LaneState<VPL> s = s0;
@@ -40,7 +40,9 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.G > 0) {
     for (int k = tp.lane; k < P.G * 24; k += 32) sm.posebar[k] = 0.0f;
   }
-  substep<VPL, true>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape);
+  ContactCache<VPL> cc;
+  cc.reset(contact_flag ? -1.0f : 1.0e30f);   // the replay saw no self-contact correction in this substep: skip it outright
+  substep<VPL, true>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc);
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
 
   f3 tbar_old[VPL], tbar_new[VPL];
@@ -115,7 +117,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.self_contact && R.any_pen) {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = k * 32 + tp.lane;
+      const int i = vpos<VPL>(tp.base + k);
       sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
       sts3(sm.vs, sm.NP, i, (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k]);
       sts3(sm.vbar, sm.NP, i, (c.kin[k] == KIN_FREE) ? velbar[k] : zero3<float>());
@@ -126,7 +128,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = k * 32 + tp.lane;
+      const int i = vpos<VPL>(tp.base + k);
       velbar[k] += lds3(sm.acc, sm.NP, i);
       ybar[k] += lds3(sm.ybar, sm.NP, i);
       sts3(sm.acc, sm.NP, i, zero3<float>());
@@ -155,7 +157,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
-        const int i = k * 32 + tp.lane;
+        const int i = vpos<VPL>(tp.base + k);
         R.dx[k] -= lds3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i);
         sts3(sm.ys, sm.NP, i, R.xp[k] + R.dx[k]);
         sts3(sm.vbar, sm.NP, i, dxb[k]);
@@ -166,7 +168,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       __syncwarp();
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
-        const f3 yb = lds3(sm.ybar, sm.NP, k * 32 + tp.lane);
+        const f3 yb = lds3(sm.ybar, sm.NP, vpos<VPL>(tp.base + k));
         dxb[k] += yb;
         xpb[k] += yb;
       }
@@ -308,7 +310,7 @@ __global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_adjoint(const __gr
   const int wib = threadIdx.x >> 5, env = blockIdx.x * DLO_WARPS_PER_BLOCK + wib;
   if (env >= P.B) return;
   WarpSmem sm;
-  sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 32 * VPL);
+  sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
   Topo<VPL> tp;
   tp.init(P);
   EnvConst<VPL> c;
@@ -329,7 +331,8 @@ __global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_adjoint(const __gr
     for (int sub = P.n_sub - 1; sub >= 0; --sub) {
       LaneState<VPL> s0;
       load_state<VPL>(P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk, tp.base, P.NS, s0);
-      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0, A, G, acc_tape);
+      const int cflag = P.tape_flag ? (int)P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] : 1;
+      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0, A, G, acc_tape, cflag);
     }
     if (P.g_actions && tp.lane < P.G) {
       float* gc = P.g_actions + (((size_t)t * P.B + env) * P.G + tp.lane) * 6;

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32, VPL <= 4 ? 3 : 2) k_
   const int wib = threadIdx.x >> 5, env = blockIdx.x * DLO_WARPS_PER_BLOCK + wib;
   if (env >= P.B) return;
   WarpSmem sm;
-  sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 32 * VPL);
+  sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
   Topo<VPL> tp;
   tp.init(P);
   EnvConst<VPL> c;
@@ -179,11 +179,14 @@ __global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32, VPL <= 4 ? 3 : 2) k_
   edge_prev_refresh<VPL>(tp, s, ec);
   float ap[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, ac[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   SubRec<VPL> R;
+  ContactCache<VPL> cc;
+  cc.reset(-1.0f);
   for (int t = t0; t < t1; ++t) {
     if (P.G > 0) load_actions(P, env, tp.lane, t, ap, ac);
     for (int sub = 0; sub < P.n_sub; ++sub) {
       if (write_tape) store_state<VPL>(P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk, tp.base, P.NS, s);
-      substep<VPL, false>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr);
+      substep<VPL, false>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
+      if (write_tape && P.tape_flag && tp.lane == 0) P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] = (uint8_t)R.any_pen;
     }
     if (stride > 0 && (t + 1) % stride == 0) store_state<VPL>(P.ckpt + ((size_t)((t + 1) / stride) * P.B + env) * blk, tp.base, P.NS, s);
   }

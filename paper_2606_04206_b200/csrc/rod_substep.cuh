@@ -9,12 +9,24 @@ namespace dlo {
 struct WarpSmem {
   float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk;
   unsigned short* cand;
-  int NP;   // 32*VPL
+  int NP;   // row stride of the per-vertex arrays: 33*VPL (32*VPL vertices + pad words, see vpos)
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
     lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk;
     NP = np;
+  }
+};
+
+// what is known about self-contact from earlier substeps: positions at which the candidate list was last built and
+// the exact minimum pair distance there (dref < 0: nothing known, build at first need; huge: never build)
+template <int VPL> struct ContactCache {
+  f3 xref[VPL];
+  float dref;
+  __device__ __forceinline__ void reset(float d) {
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) xref[k] = zero3<float>();
+    dref = d;
   }
 };
 
@@ -89,13 +101,13 @@ __device__ __forceinline__ void bending_forces(const Topo<VPL>& tp, const LaneSt
   }
 }
 
-// segment-pair test used by the candidate build: exact closest distance below `lim` (pa.. are smem positions)
-__device__ __forceinline__ bool pair_within(const float* ys, int NP, int pa, int pan, int pb, int pbn, float lim) {
+// squared segment-segment distance of an edge pair (pa.. are smem positions of the four end points)
+__device__ __forceinline__ float pair_dist2(const float* ys, int NP, int pa, int pan, int pb, int pbn) {
   f3 p1 = lds3(ys, NP, pa), q1 = lds3(ys, NP, pan), p2 = lds3(ys, NP, pb), q2 = lds3(ys, NP, pbn);
   float t, u;
   closest_points<float>(p1, q1, p2, q2, t, u);
   f3 dv = axpy(p1, t, q1 - p1) - axpy(p2, u, q2 - p2);
-  return dot(dv, dv) < lim * lim;
+  return dot(dv, dv);
 }
 
 // A4 candidate list (Eq.13 "potentially colliding", R-15): all edge pairs a<b with cyclic index distance >=
@@ -105,8 +117,9 @@ __device__ __forceinline__ bool pair_within(const float* ys, int NP, int pa, int
 // survivors take the exact segment-segment test, 32 at a time.  Every rejection is conservative, so no pair is
 // lost.  Order: by (block a, block b, slot a, slot b) - deterministic, but not the oracle's lexicographic order
 // (only the fp32 summation order of the Jacobi pass depends on it).  ys = x^p, mid = (midpoint, half length, w).
+struct CandOut { int ncand; float dmin; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b)
 template <int VPL>
-__device__ __noinline__ int build_candidates(const KParams& P, int lane, const WarpSmem& sm, int env, float bx, float by, float bz, float br) {
+__device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, const WarpSmem& sm, int env, float bx, float by, float bz, float br) {
   const int E = P.E, N = P.N, NP = sm.NP, nb = (E + VPL - 1) / VPL;
   const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
   constexpr int PP = VPL * VPL, NPER = PP <= 32 ? 32 / PP : 1, ITER = (PP + 31) / 32;
@@ -129,11 +142,13 @@ __device__ __noinline__ int build_candidates(const KParams& P, int lane, const W
 #pragma unroll
       for (int j = 0; j < ITER; ++j) {
         const int sub = (PP <= 32) ? lane / PP : 0, idx = (PP <= 32) ? lane % PP : j * 32 + lane;
-        const unsigned Bsel = __fns(mask, 0, sub + 1);
+        unsigned mm = mask, Bsel = 0xffffffffu;   // the (sub+1)-th set bit of mask
+#pragma unroll
+        for (int q = 0; q < NPER; ++q) { if (q == sub && mm) Bsel = __ffs(mm) - 1; mm &= mm - 1u; }
         const int ka = idx / VPL, kb = idx % VPL, a = A * VPL + ka, b = (int)Bsel * VPL + kb, d = b - a;
         bool hit = false;
         if (Bsel != 0xffffffffu && idx < PP && sub < NPER && b < E && d >= P.self_skip && (!P.ring || E - d >= P.self_skip)) {
-          const int pa = ka * 32 + A, pb = kb * 32 + (int)Bsel;
+          const int pa = vpos<VPL>(a), pb = vpos<VPL>(b);
           const float dx = sm.mid[pb] - sm.mid[pa], dy = sm.mid[NP + pb] - sm.mid[NP + pa], dz = sm.mid[2 * NP + pb] - sm.mid[2 * NP + pa];
           const float reach = sm.mid[3 * NP + pa] + sm.mid[3 * NP + pb] + lim;
           hit = dx * dx + dy * dy + dz * dz < reach * reach;
@@ -154,6 +169,7 @@ __device__ __noinline__ int build_candidates(const KParams& P, int lane, const W
   __syncwarp();
   // (3) exact narrow phase on the survivors, ordered compaction into the candidate list
   int ncand = 0;
+  float d2min = lim * lim;
   for (int p0 = 0; p0 < nsurv; p0 += 32) {
     const int p = p0 + lane;
     bool hit = false;
@@ -161,7 +177,9 @@ __device__ __noinline__ int build_candidates(const KParams& P, int lane, const W
     if (p < nsurv) {
       c = surv[p];
       const int a = c >> 8, b = c & 255, an = (a + 1 < N) ? a + 1 : 0, bn = (b + 1 < N) ? b + 1 : 0;
-      hit = pair_within(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn), lim);
+      const float d2 = pair_dist2(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn));
+      hit = d2 < lim * lim;
+      d2min = fminf(d2min, d2);
     }
     const unsigned m = __ballot_sync(DLO_FULL, hit);
     if (hit) sm.cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)c;
@@ -169,7 +187,10 @@ __device__ __noinline__ int build_candidates(const KParams& P, int lane, const W
   }
   if (overflow && lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
   __syncwarp();
-  return ncand;
+  CandOut out;
+  out.ncand = ncand;
+  out.dmin = overflow ? 0.0f : sqrt_(warp_min(d2min));
+  return out;
 }
 
 // serialised (deterministic, candidate-order) accumulation of one lane's four vertex contributions
@@ -315,7 +336,7 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
 template <int VPL, bool REC>
 __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                         const float ap[6], const float ac[6], int sub, LaneState<VPL>& s, EdgeCache<VPL>& ec,
-                                        SubRec<VPL>& R, float* acc_tape) {
+                                        SubRec<VPL>& R, float* acc_tape, ContactCache<VPL>& cc) {
   const float h = P.h, inv_h = P.inv_h;
   // -- A1 bodies
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);
@@ -355,14 +376,27 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
 #pragma unroll
   for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
 
+  // Self-contact is evaluated lazily (exactly): segment distance is 1-Lipschitz in the end points, so with d_ref the
+  // minimum pair distance at the positions x_ref where the candidate list was last built, no pair can penetrate
+  // while d_ref - 2 (max_i |x^p_i - x_ref,i| + max_i |dx_i|) >= r_a + r_b.  Only when that bound fails is the list
+  // (re)built at x^p and the Jacobi pass run.  A pass that cannot apply a correction changes nothing, so the
+  // state is identical to building and sweeping every time.
   R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
+  bool built = false;
+  float D1 = 0.0f;
   if (P.self_contact) {
+    float m2 = 0.0f;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.vvalid[k]) { const f3 d = R.xp[k] - cc.xref[k]; m2 = fmaxf(m2, dot(d, d)); }
+    D1 = sqrt_(warp_max(m2));
+  }
+  auto build_list = [&]() {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = k * 32 + tp.lane;   // own vertex, slot-major position
+      const int i = vpos<VPL>(tp.base + k);
       sts3(sm.ys, sm.NP, i, R.xp[k]);
-      f3 mid = axpy(R.xp[k], 0.5f, epred[k]);
-      sts3(sm.mid, sm.NP, i, mid);
+      sts3(sm.mid, sm.NP, i, axpy(R.xp[k], 0.5f, epred[k]));
       sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
       sm.mid[4 * sm.NP + i] = c.w[k];
     }
@@ -382,10 +416,14 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         }
     }
     __syncwarp();
-    R.ncand = build_candidates<VPL>(P, tp.lane, sm, env, bc.x, bc.y, bc.z, brad);
+    const CandOut co = build_candidates<VPL>(P, tp.lane, sm, env, bc.x, bc.y, bc.z, brad);
+    R.ncand = co.ncand;
+    cc.dref = co.dmin;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) cc.xref[k] = R.xp[k];
     for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
     __syncwarp();
-  }
+  };
 
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
@@ -448,9 +486,23 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         if (REC) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
       }
     }
-    if (P.self_contact && R.ncand > 0) {
+    bool sweep = false;
+    if (P.self_contact) {
+      float m2 = 0.0f;
 #pragma unroll
-      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, k * 32 + tp.lane, R.xp[k] + R.dx[k]);
+      for (int k = 0; k < VPL; ++k) m2 = fmaxf(m2, dot(R.dx[k], R.dx[k]));
+      const float Dm = sqrt_(warp_max(m2)), need = 2.0f * P.r + 1.0e-6f;
+      sweep = !(cc.dref - 2.0f * (D1 + Dm) >= need);
+      if (sweep && !built) {
+        build_list();
+        built = true;
+        D1 = 0.0f;
+        sweep = !(cc.dref - 2.0f * Dm >= need);
+      }
+    }
+    if (sweep && R.ncand > 0) {
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]);
       __syncwarp();
       const bool any = contact_pass<VPL>(P, tp, sm, R.ncand, c.inv_m);
       __syncwarp();
@@ -459,7 +511,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         R.jac_mask |= 1u << it;
 #pragma unroll
         for (int k = 0; k < VPL; ++k) {
-          const int i = k * 32 + tp.lane;   // own vertex, slot-major position
+          const int i = vpos<VPL>(tp.base + k);   // own vertex, slot-major position
           const f3 a = lds3(sm.acc, sm.NP, i);
           R.dx[k] += a;
           if (REC) sts3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i, a);
@@ -476,13 +528,13 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) vel[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k];
   if (P.self_contact && R.any_pen) {
 #pragma unroll
-    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, k * 32 + tp.lane, R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, k * 32 + tp.lane, vel[k]); }
+    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, vpos<VPL>(tp.base + k), vel[k]); }
     __syncwarp();
     friction_pass<VPL>(P, tp, sm, R.ncand, c.mu_s);
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const int i = k * 32 + tp.lane;   // own vertex, slot-major position
+      const int i = vpos<VPL>(tp.base + k);   // own vertex, slot-major position
       if (c.kin[k] == KIN_FREE) vel[k] += lds3(sm.acc, sm.NP, i);
       sts3(sm.acc, sm.NP, i, zero3<float>());
     }

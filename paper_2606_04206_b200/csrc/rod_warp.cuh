@@ -42,6 +42,7 @@ struct KParams {
   float* acc_tape;       // [B][N_C][3][32*VPL] self-contact corrections of the substep being reversed
   float* gmat;           // [B][5] running material gradient
   float* g_actions;      // [H][B][G][6] (may be null)
+  uint8_t* tape_flag;    // [stride*n_sub][B]: 1 if the substep applied a self-contact correction (written by the replay)
   // per-warp shared memory layout (float offsets from the warp's base), set by the host
   int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_blk, sm_warp_floats;
 };
@@ -56,9 +57,19 @@ __device__ __forceinline__ float warp_sum(float v) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(DLO_FULL, v, o);
   return v;
 }
-// shared-memory position of vertex i: slot-major ((i % VPL) * 32 + i / VPL), so that the lanes' own vertices
-// (slot k of lane l -> k*32 + l) are bank-conflict free; random access by vertex index goes through vpos()
-template <int VPL> __device__ __forceinline__ int vpos(int i) { return (i % VPL) * 32 + i / VPL; }
+// shared-memory position of vertex i: natural order plus one pad word per 32, so that both access patterns are
+// bank-conflict free: the lanes' own vertices (stride VPL across lanes) and runs of consecutive vertices (candidates)
+template <int VPL> __device__ __forceinline__ int vpos(int i) { return i + (i >> 5); }
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(DLO_FULL, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(DLO_FULL, v, o));
+  return v;
+}
 __device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
 __device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
 
