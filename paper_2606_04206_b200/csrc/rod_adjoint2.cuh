@@ -50,6 +50,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 #pragma unroll
   for (int k = 0; k < VPL; ++k) { tbar_old[k] = zero3<float>(); tbar_new[k] = zero3<float>(); iLbar_old[k] = 0.0f; }
 
+  phase_sync(sm);
   // ---- reverse A9: plasticity (Eq.11), then the frame transport
   if (P.plasticity) {
     const float Y = c.sigy * c.l0;
@@ -91,6 +92,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.x[0] += shfl3(send, tp.pl);
   }
 
+  phase_sync(sm);
   // ---- reverse A8 commit
   f3 velbar[VPL];
 #pragma unroll
@@ -101,6 +103,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.v[k] = zero3<float>();
   }
 
+  phase_sync(sm);
   // ---- reverse A7 rigid coupling
   f3 ybar[VPL];
 #pragma unroll
@@ -109,6 +112,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (c.kin[k] == KIN_FREE && R.active[k]) rigid_coupling_adj(P, sm, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k], ybar[k]);
   }
 
+  phase_sync(sm);
   // ---- reverse A6 friction + reconciliation.  velbar is now the adjoint of v^3.
   if (P.self_contact && R.ncand > 0) {
     for (int p = tp.lane; p < R.ncand; p += 32) sm.dpbar[p] = 0.0f;
@@ -146,6 +150,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     Sb[k] = 0.0f;
   }
 
+  phase_sync(sm);
   // ---- reverse A5: iterations backwards; each Eq.10 update is undone from its stored multiplier
   const f3 xpr = shfl3(R.xp[0], tp.nl);
   f3 epred[VPL];
@@ -154,6 +159,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   const float atil = c.stretch * inv_h * inv_h;
   float atilbar = 0.0f;
   for (int it = P.N_C - 1; it >= 0; --it) {
+    phase_sync(sm);
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
@@ -220,6 +226,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     xpb[0] += shfl3(send, tp.pl);
   }
 
+  phase_sync(sm);
   // ---- reverse A4 predict, A3 velocity
   const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
   f3 fbar[VPL];
@@ -239,6 +246,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     }
   }
 
+  phase_sync(sm);
   // ---- reverse A2 forces: bending elements (and the stretch force in ENERGY mode) -> old edge geometry
   {
     const f3 fb_prev = shfl3(pick_last<VPL>(fbar, tp.ks), tp.pl), fb_next = shfl3(fbar[0], tp.nl);
@@ -285,6 +293,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.x[0] += shfl3(send, tp.pl);
   }
 
+  phase_sync(sm);
   // ---- reverse A1: pose adjoints -> action adjoints (lane g owns gripper g)
   if (P.G > 0) {
     __syncwarp();
@@ -311,6 +320,7 @@ __global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_adjoint(const __gr
   if (env >= P.B) return;
   WarpSmem sm;
   sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
+  sm.sync_threads = 32 * min(DLO_WARPS_PER_BLOCK, P.B - (int)blockIdx.x * DLO_WARPS_PER_BLOCK);
   Topo<VPL> tp;
   tp.init(P);
   EnvConst<VPL> c;

@@ -9,14 +9,22 @@ namespace dlo {
 struct WarpSmem {
   float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk;
   unsigned short* cand;
+  int sync_threads;   // > 0: warps of the CTA walk the phases in lockstep (named barrier over this many threads)
   int NP;   // row stride of the per-vertex arrays: 33*VPL (32*VPL vertices + pad words, see vpos)
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
     lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk;
     NP = np;
+    sync_threads = 0;
   }
 };
+
+// Phase barrier of the big kernels.  All warps of a CTA run the same long instruction stream on different envs; kept
+// in step, one instruction-cache fill serves all of them.  Must only be called from CTA-uniform control flow.
+__device__ __forceinline__ void phase_sync(const WarpSmem& sm) {
+  if (sm.sync_threads > 0) asm volatile("bar.sync 1, %0;" ::"r"(sm.sync_threads) : "memory");
+}
 
 // what is known about self-contact from earlier substeps: positions at which the candidate list was last built and
 // the exact minimum pair distance there (dref < 0: nothing known, build at first need; huge: never build)
@@ -341,6 +349,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // -- A1 bodies
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);
 
+  phase_sync(sm);
   // -- A2 forces: gravity, stretch (mode ENERGY, Eq.2-3), bending (Eq.4-7)
   f3 f[VPL];
 #pragma unroll
@@ -358,6 +367,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   }
   bending_forces<VPL>(tp, s, ec, c.alpha / c.l0, f);
 
+  phase_sync(sm);
   // -- A3 velocity (symplectic Euler L97, implicit viscous damping R-7), A4 predict
   const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
 #pragma unroll
@@ -425,9 +435,11 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     __syncwarp();
   };
 
+  phase_sync(sm);
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
   for (int it = 0; it < P.N_C; ++it) {
+    phase_sync(sm);
     if (P.stretch_mode == 1) {
       // red: even slots, both end points local
 #pragma unroll
@@ -522,6 +534,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     }
   }
 
+  phase_sync(sm);
   // -- A6 reconcile v with the projected positions (R-11) + self-contact friction
   f3 vel[VPL];
 #pragma unroll
@@ -541,6 +554,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     __syncwarp();
   }
 
+  phase_sync(sm);
   // -- A7 rigid soft coupling at y = x^p + dx
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
@@ -553,6 +567,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     R.v4[k] = vel[k];
   }
 
+  phase_sync(sm);
   // -- A8 commit
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
@@ -561,6 +576,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     else if (tp.vvalid[k]) s.v[k] = zero3<float>();
   }
 
+  phase_sync(sm);
   // -- A9 frames: time-parallel transport (R-4), then plasticity (Eq.11)
   edge_refresh<VPL>(tp, s, ec);
 #pragma unroll
