@@ -6,6 +6,7 @@
 #include <string.h>
 #include <string>
 #include <vector>
+#include <algorithm>
 
 #include "../../include/dlo.h"
 #include "rod_kernels.cuh"
@@ -28,7 +29,8 @@ struct dlo_sim {
   dlo_config cfg;
   cudaStream_t stream;
   KParams P;                      // kernel parameter block (pointers filled as buffers appear)
-  int VPL, smem_fwd, smem_adj;
+  int VPL, smem_fwd, smem_adj;    // dynamic shared memory per CTA
+  int wpb_fwd, wpb_adj;           // warps (envs) per CTA
   size_t blk;                     // floats per env state block
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
@@ -70,7 +72,7 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
     if (P.self_contact) { P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP); }
   }
   P.sm_warp_floats = o;
-  return o * (int)sizeof(float) * DLO_WARPS_PER_BLOCK;
+  return o * (int)sizeof(float);   // bytes per warp
 }
 
 static dlo_status validate(const dlo_config* c) {
@@ -147,10 +149,17 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   KParams& P = s->P;
   s->VPL = vpl_for(P.N);
   s->blk = (size_t)STATE_ROWS * P.NS;
-  s->smem_fwd = smem_layout(P, s->VPL, false);
-  KParams Pa = P;
-  s->smem_adj = smem_layout(Pa, s->VPL, true);
-  if (s->smem_adj > 227 * 1024) { delete s; return fail(DLO_ERR_UNSUPPORTED, "shared memory per block exceeds 227 KB for this n_verts / n_proj_iters"); }
+  {
+    const int per_fwd = smem_layout(P, s->VPL, false);
+    KParams Pa = P;
+    const int per_adj = smem_layout(Pa, s->VPL, true);
+    const int cap = 227 * 1024;
+    if (per_adj > cap) { delete s; return fail(DLO_ERR_UNSUPPORTED, "shared memory per env exceeds 227 KB for this n_verts / n_proj_iters"); }
+    s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, (cap / 2) / std::max(per_fwd, 1)));   // two CTAs per SM
+    s->wpb_adj = std::max(1, std::min(DLO_ADJ_WARPS, cap / std::max(per_adj, 1)));
+    s->smem_fwd = per_fwd * s->wpb_fwd;
+    s->smem_adj = per_adj * s->wpb_adj;
+  }
   const size_t B = P.B;
 #define CUD(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { dlo_destroy(s); return fail(e_ == cudaErrorMemoryAllocation ? DLO_ERR_OOM : DLO_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); } } while (0)
   CUD(dalloc(&s->mat, B * MAT_N));
@@ -271,8 +280,8 @@ template <int VPL> static cudaError_t launch_forward_t(dlo_sim* s, int t0, int t
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  const int grid = (s->P.B + DLO_WARPS_PER_BLOCK - 1) / DLO_WARPS_PER_BLOCK;
-  k_forward<VPL><<<grid, DLO_WARPS_PER_BLOCK * 32, s->smem_fwd, s->stream>>>(s->P, t0, t1, stride, write_tape);
+  const int grid = (s->P.B + s->wpb_fwd - 1) / s->wpb_fwd;
+  k_forward<VPL><<<grid, s->wpb_fwd * 32, s->smem_fwd, s->stream>>>(s->P, t0, t1, stride, write_tape);
   s->launches += 1;
   return cudaGetLastError();
 }

@@ -3,8 +3,8 @@
 template <int VPL> static cudaError_t launch_adjoint_t(dlo_sim* s, const KParams& P, int t0, int t1) {
   cudaError_t e = cudaFuncSetAttribute(k_adjoint<VPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_adj > 48 * 1024 ? s->smem_adj : 48 * 1024);
   if (e != cudaSuccess) return e;
-  const int grid = (P.B + DLO_WARPS_PER_BLOCK - 1) / DLO_WARPS_PER_BLOCK;
-  k_adjoint<VPL><<<grid, DLO_WARPS_PER_BLOCK * 32, s->smem_adj, s->stream>>>(P, t0, t1);
+  const int grid = (P.B + s->wpb_adj - 1) / s->wpb_adj;
+  k_adjoint<VPL><<<grid, s->wpb_adj * 32, s->smem_adj, s->stream>>>(P, t0, t1);
   s->launches += 1;
   return cudaGetLastError();
 }

@@ -314,13 +314,13 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 // Segment adjoint: walks the substeps of steps t1-1 .. t0 backwards, one warp per env.  P.tape holds the state at
 // the start of every substep of the segment (written by k_forward), P.adj the running state adjoint.
 template <int VPL>
-__global__ void __launch_bounds__(DLO_WARPS_PER_BLOCK * 32) k_adjoint(const __grid_constant__ KParams P, int t0, int t1) {
+__global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_constant__ KParams P, int t0, int t1) {
   extern __shared__ __align__(16) float smem[];
-  const int wib = threadIdx.x >> 5, env = blockIdx.x * DLO_WARPS_PER_BLOCK + wib;
+  const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
   if (env >= P.B) return;
   WarpSmem sm;
   sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
-  sm.sync_threads = 32 * min(DLO_WARPS_PER_BLOCK, P.B - (int)blockIdx.x * DLO_WARPS_PER_BLOCK);
+  sm.sync_threads = 32 * min(wpb, P.B - (int)blockIdx.x * wpb);
   Topo<VPL> tp;
   tp.init(P);
   EnvConst<VPL> c;
