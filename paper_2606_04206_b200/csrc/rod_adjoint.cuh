@@ -81,8 +81,12 @@ __device__ __forceinline__ bool body_eval(const KParams& P, const WarpSmem& sm, 
 
 // reverse of A7 for one free vertex: `active` = bodies that responded (forward order = bit order), v3 = velocity
 // before the coupling.  velbar: in = adjoint of v4, out = adjoint of v3.  ybar += adjoint of y.
-__device__ __noinline__ void rigid_coupling_adj(const KParams& P, const WarpSmem& sm, int env, unsigned active, const f3& y, const f3& v3,
-                                                float mu_r, f3& velbar, f3& ybar) {
+struct CoupleAdj { f3 velbar, ybar; };
+__device__ __noinline__ CoupleAdj rigid_coupling_adj(const KParams& P, float* smbase, int np, int env, unsigned active, f3 y, f3 v3, float mu_r,
+                                                     f3 velbar) {
+  WarpSmem sm;
+  sm.init(P, smbase, np);
+  f3 ybar = zero3<float>();
   unsigned m = active;
   while (m) {
     const int b = 31 - __clz(m);
@@ -121,6 +125,9 @@ __device__ __noinline__ void rigid_coupling_adj(const KParams& P, const WarpSmem
       posebar_add(sm.posebar + g * 24 + 12, b1);
     }
   }
+  CoupleAdj out;
+  out.velbar = velbar; out.ybar = ybar;
+  return out;
 }
 
 // serialised scatter of four vertex adjoints (positions -> ybar, optionally velocities -> acc)
@@ -144,11 +151,13 @@ template <int VPL> __device__ __forceinline__ void cand_verts(const WarpSmem& sm
 
 // reverse of one Eq.13 Jacobi pass: positions y (before the pass) in sm.ys, adjoint of the post-pass corrections
 // in sm.vbar, adjoint of D_p in sm.dpbar; position adjoints are summed into sm.ybar
-template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand) {
+template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& P, int lane, float* smbase, int ncand) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
   const float rsum = 2.0f * P.r;
   for (int p0 = 0; p0 < ncand; p0 += 32) {
-    const int p = p0 + tp.lane;
+    const int p = p0 + lane;
     bool hit = false;
     int iv[4] = {0, 0, 0, 0};
     f3 xb[4] = {zero3<float>(), zero3<float>(), zero3<float>(), zero3<float>()};
@@ -163,16 +172,18 @@ template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& 
       const float reach = 0.5f * (sqrt_(dot(ea, ea)) + sqrt_(dot(eb, eb))) + rsum;
       if (dot(dm, dm) < reach * reach) hit = contact_adj<float>(xs, ws, rsum, ob, sm.dpbar[p], xb);
     }
-    ordered_scatter_vec4(__ballot_sync(DLO_FULL, hit), tp.lane, sm.ybar, NP, iv, xb);
+    ordered_scatter_vec4(__ballot_sync(DLO_FULL, hit), lane, sm.ybar, NP, iv, xb);
   }
 }
 
 // reverse of the friction pass: y in sm.ys, v^2 in sm.vs, adjoint of v^3 in sm.vbar; writes sm.dpbar, sums
 // position adjoints into sm.ybar and velocity adjoints into sm.acc
-template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand, float mu_s) {
+template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams& P, int lane, float* smbase, int ncand, float mu_s) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
   for (int p0 = 0; p0 < ncand; p0 += 32) {
-    const int p = p0 + tp.lane;
+    const int p = p0 + lane;
     bool hit = false;
     int iv[4] = {0, 0, 0, 0};
     f3 xb[4] = {zero3<float>(), zero3<float>(), zero3<float>(), zero3<float>()};
@@ -188,8 +199,8 @@ template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams&
       sm.dpbar[p] = dpb;
     }
     const unsigned hits = __ballot_sync(DLO_FULL, hit);
-    ordered_scatter_vec4(hits, tp.lane, sm.ybar, NP, iv, xb);
-    ordered_scatter_vec4(hits, tp.lane, sm.acc, NP, iv, vb);
+    ordered_scatter_vec4(hits, lane, sm.ybar, NP, iv, xb);
+    ordered_scatter_vec4(hits, lane, sm.acc, NP, iv, vb);
   }
 }
 

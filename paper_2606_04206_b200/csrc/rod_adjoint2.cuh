@@ -109,7 +109,10 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
     ybar[k] = zero3<float>();
-    if (c.kin[k] == KIN_FREE && R.active[k]) rigid_coupling_adj(P, sm, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k], ybar[k]);
+    if (c.kin[k] == KIN_FREE && R.active[k]) {
+      const CoupleAdj ca = rigid_coupling_adj(P, sm.base, sm.NP, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k]);
+      velbar[k] = ca.velbar; ybar[k] = ca.ybar;
+    }
   }
 
   phase_sync(sm);
@@ -128,7 +131,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       sts3(sm.ybar, sm.NP, i, zero3<float>());
     }
     __syncwarp();
-    friction_pass_adj<VPL>(P, tp, sm, R.ncand, c.mu_s);
+    friction_pass_adj<VPL>(P, tp.lane, sm.base, R.ncand, c.mu_s);
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
@@ -159,7 +162,6 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   const float atil = c.stretch * inv_h * inv_h;
   float atilbar = 0.0f;
   for (int it = P.N_C - 1; it >= 0; --it) {
-    phase_sync(sm);
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
@@ -170,7 +172,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         sts3(sm.ybar, sm.NP, i, zero3<float>());
       }
       __syncwarp();
-      contact_pass_adj<VPL>(P, tp, sm, R.ncand);
+      contact_pass_adj<VPL>(P, tp.lane, sm.base, R.ncand);
       __syncwarp();
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {

@@ -9,6 +9,7 @@ namespace dlo {
 struct WarpSmem {
   float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk;
   unsigned short* cand;
+  float* base;        // the warp's shared-memory block (non-inlined helpers rebuild the view from this one pointer)
   int sync_threads;   // > 0: warps of the CTA walk the phases in lockstep (named barrier over this many threads)
   int NP;   // row stride of the per-vertex arrays: 33*VPL (32*VPL vertices + pad words, see vpos)
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
@@ -16,6 +17,7 @@ struct WarpSmem {
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
     lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk;
     NP = np;
+    this->base = base;
     sync_threads = 0;
   }
 };
@@ -127,7 +129,9 @@ __device__ __forceinline__ float pair_dist2(const float* ys, int NP, int pa, int
 // (only the fp32 summation order of the Jacobi pass depends on it).  ys = x^p, mid = (midpoint, half length, w).
 struct CandOut { int ncand; float dmin; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b)
 template <int VPL>
-__device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, const WarpSmem& sm, int env, float bx, float by, float bz, float br) {
+__device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, float* smbase, int env, float bx, float by, float bz, float br) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
   const int E = P.E, N = P.N, NP = sm.NP, nb = (E + VPL - 1) / VPL;
   const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
   constexpr int PP = VPL * VPL, NPER = PP <= 32 ? 32 / PP : 1, ITER = (PP + 31) / 32;
@@ -219,12 +223,14 @@ __device__ __forceinline__ void ordered_scatter4(unsigned hits, int lane, float*
 // A5(ii): one Jacobi pass of Eq.13 over the candidates at y (in sm.ys); corrections summed into sm.acc, D_p += d.
 // Returns true if any correction was applied.
 template <int VPL>
-__device__ bool contact_pass(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand, float inv_m) {
+__device__ __noinline__ bool contact_pass(const KParams& P, int lane, float* smbase, int ncand) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
   const float rsum = 2.0f * P.r;
   bool any = false;
   for (int p0 = 0; p0 < ncand; p0 += 32) {
-    const int p = p0 + tp.lane;
+    const int p = p0 + lane;
     bool hit = false;
     int iv[4] = {0, 0, 0, 0};
     float coef[4] = {0.f, 0.f, 0.f, 0.f};
@@ -254,18 +260,19 @@ __device__ bool contact_pass(const KParams& P, const Topo<VPL>& tp, const WarpSm
     }
     const unsigned hits = __ballot_sync(DLO_FULL, hit);
     any |= hits != 0u;
-    ordered_scatter4(hits, tp.lane, sm.acc, NP, iv, coef, n);
+    ordered_scatter4(hits, lane, sm.acc, NP, iv, coef, n);
   }
-  (void)inv_m;
   return any;
 }
 
 // A6 self-contact friction (L410, R-16) for candidates with D_p > 0: velocities in sm.vs, positions in sm.ys
 template <int VPL>
-__device__ void friction_pass(const KParams& P, const Topo<VPL>& tp, const WarpSmem& sm, int ncand, float mu_s) {
+__device__ __noinline__ void friction_pass(const KParams& P, int lane, float* smbase, int ncand, float mu_s) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
   for (int p0 = 0; p0 < ncand; p0 += 32) {
-    const int p = p0 + tp.lane;
+    const int p = p0 + lane;
     bool hit = false;
     int iv[4] = {0, 0, 0, 0};
     float coef[4] = {0.f, 0.f, 0.f, 0.f};
@@ -301,7 +308,7 @@ __device__ void friction_pass(const KParams& P, const Topo<VPL>& tp, const WarpS
       }
     }
     const unsigned hits = __ballot_sync(DLO_FULL, hit);
-    ordered_scatter4(hits, tp.lane, sm.acc, NP, iv, coef, D);
+    ordered_scatter4(hits, lane, sm.acc, NP, iv, coef, D);
   }
 }
 
@@ -426,7 +433,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         }
     }
     __syncwarp();
-    const CandOut co = build_candidates<VPL>(P, tp.lane, sm, env, bc.x, bc.y, bc.z, brad);
+    const CandOut co = build_candidates<VPL>(P, tp.lane, sm.base, env, bc.x, bc.y, bc.z, brad);
     R.ncand = co.ncand;
     cc.dref = co.dmin;
 #pragma unroll
@@ -439,7 +446,6 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
   for (int it = 0; it < P.N_C; ++it) {
-    phase_sync(sm);
     if (P.stretch_mode == 1) {
       // red: even slots, both end points local
 #pragma unroll
@@ -516,7 +522,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
 #pragma unroll
       for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]);
       __syncwarp();
-      const bool any = contact_pass<VPL>(P, tp, sm, R.ncand, c.inv_m);
+      const bool any = contact_pass<VPL>(P, tp.lane, sm.base, R.ncand);
       __syncwarp();
       if (any) {
         R.any_pen = 1;
@@ -543,7 +549,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
 #pragma unroll
     for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, vpos<VPL>(tp.base + k), vel[k]); }
     __syncwarp();
-    friction_pass<VPL>(P, tp, sm, R.ncand, c.mu_s);
+    friction_pass<VPL>(P, tp.lane, sm.base, R.ncand, c.mu_s);
     __syncwarp();
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
