@@ -27,10 +27,13 @@ __device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float w
 // out = adjoint of the state at its start.  G accumulates material / action adjoints of this lane.
 template <int VPL>
 __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
-                                                const float ap[6], const float ac[6], int sub, const LaneState<VPL>& s0,
+                                                const float ap[6], const float ac[6], int sub, const float* __restrict__ s0blk,
                                                 LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag) {
   const float h = P.h, inv_h = P.inv_h;
-  // ---- forward recompute with recording
+  // ---- forward recompute with recording.  The start state is read from the tape twice (here and again for the
+  // reverse of A2) rather than held in ~70 registers across the projection loop, the hottest part of the kernel.
+  LaneState<VPL> s0;
+  load_state<VPL>(s0blk, tp.base, P.NS, s0);
   LaneState<VPL> s = s0;
   EdgeCache<VPL> ec0, ec;
   edge_refresh<VPL>(tp, s0, ec0);
@@ -46,9 +49,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
 
   f3 tbar_old[VPL], tbar_new[VPL];
-  float iLbar_old[VPL];
 #pragma unroll
-  for (int k = 0; k < VPL; ++k) { tbar_old[k] = zero3<float>(); tbar_new[k] = zero3<float>(); iLbar_old[k] = 0.0f; }
+  for (int k = 0; k < VPL; ++k) { tbar_old[k] = zero3<float>(); tbar_new[k] = zero3<float>(); }
 
   phase_sync(sm);
   // ---- reverse A9: plasticity (Eq.11), then the frame transport
@@ -101,6 +103,14 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (c.kin[k] == KIN_FREE) velbar[k] = axpy(A.v[k], h, A.x[k]);
     else if (c.kin[k] >= KIN_GRASP0) { grasp_target_adj(P, sm, c.kin[k], A.x[k]); velbar[k] = A.v[k]; A.x[k] = zero3<float>(); }
     A.v[k] = zero3<float>();
+  }
+
+  {   // old tangents (frame transport) -> old positions, while the old edge geometry is still at hand
+    f3 send = zero3<float>();
+#pragma unroll
+    for (int k = 0; k < VPL; ++k)
+      if (tp.evalid[k]) scatter_edge<VPL>(A.x, send, k, tp.ks, normalize_adj<float>(ec0.t[k], ec0.iL[k], tbar_old[k], 0.0f));
+    A.x[0] += shfl3(send, tp.pl);
   }
 
   phase_sync(sm);
@@ -230,6 +240,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 
   phase_sync(sm);
   // ---- reverse A4 predict, A3 velocity
+  LaneState<VPL> s0b;
+  load_state<VPL>(s0blk, tp.base, P.NS, s0b);
   const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
   f3 fbar[VPL];
 #pragma unroll
@@ -240,7 +252,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (c.kin[k] == KIN_FREE) {
       A.v[k] = idamp * v1bar[k];
       fbar[k] = (hm * idamp) * v1bar[k];
-      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], R.v1[k]);
+      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], inv_h * (R.xp[k] - s0b.x[k]));   // v^1 = (x^p - x)/h
     } else if (c.kin[k] >= KIN_GRASP0) {
       const f3 tb = inv_h * v1bar[k];
       grasp_target_adj(P, sm, c.kin[k], tb);
@@ -251,6 +263,13 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   phase_sync(sm);
   // ---- reverse A2 forces: bending elements (and the stretch force in ENERGY mode) -> old edge geometry
   {
+    EdgeCache<VPL> eb0;
+    edge_refresh<VPL>(tp, s0b, eb0);
+    edge_prev_refresh<VPL>(tp, s0b, eb0);
+    f3 tb2[VPL];
+    float ib2[VPL];
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) { tb2[k] = zero3<float>(); ib2[k] = 0.0f; }
     const f3 fb_prev = shfl3(pick_last<VPL>(fbar, tp.ks), tp.pl), fb_next = shfl3(fbar[0], tp.nl);
     const float sc = c.alpha / c.l0;
     f3 ptb = zero3<float>(), pdb = zero3<float>();
@@ -258,40 +277,40 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
       if (tp.interior[k]) {
-        const f3 ta = (k == 0) ? ec0.pt : ec0.t[k > 0 ? k - 1 : 0];
-        const f3 da = (k == 0) ? ec0.pd1 : s0.d1[k > 0 ? k - 1 : 0];
-        const float ia = (k == 0) ? ec0.piL : ec0.iL[k > 0 ? k - 1 : 0];
+        const f3 ta = (k == 0) ? eb0.pt : eb0.t[k > 0 ? k - 1 : 0];
+        const f3 da = (k == 0) ? eb0.pd1 : s0b.d1[k > 0 ? k - 1 : 0];
+        const float ia = (k == 0) ? eb0.piL : eb0.iL[k > 0 ? k - 1 : 0];
         const f3 Gab = ((k == 0) ? fb_prev : fbar[k > 0 ? k - 1 : 0]) - fbar[k];
         const f3 Gbb = fbar[k] - next_of<VPL>(fbar, fb_next, k, tp.ks);
         f3 tab = zero3<float>(), tbb = zero3<float>(), dab = zero3<float>(), dbb = zero3<float>();
         float iab = 0.f, ibb = 0.f;
-        bend_element_adj<float>(ta, ec0.t[k], ia, ec0.iL[k], da, s0.d1[k], s0.kb1[k], s0.kb2[k], sc, Gab, Gbb, tab, tbb, iab, ibb, dab, dbb,
+        bend_element_adj<float>(ta, eb0.t[k], ia, eb0.iL[k], da, s0b.d1[k], s0b.kb1[k], s0b.kb2[k], sc, Gab, Gbb, tab, tbb, iab, ibb, dab, dbb,
                                 A.kb1[k], A.kb2[k], sbar);
-        tbar_old[k] += tbb; iLbar_old[k] += ibb; A.d1[k] += dbb;
+        tb2[k] += tbb; ib2[k] += ibb; A.d1[k] += dbb;
         if (k == 0) { ptb += tab; pdb += dab; piLb += iab; }
-        else { tbar_old[k > 0 ? k - 1 : 0] += tab; A.d1[k > 0 ? k - 1 : 0] += dab; iLbar_old[k > 0 ? k - 1 : 0] += iab; }
+        else { tb2[k > 0 ? k - 1 : 0] += tab; A.d1[k > 0 ? k - 1 : 0] += dab; ib2[k > 0 ? k - 1 : 0] += iab; }
       }
     }
     G.gm[GM_ALPHA] += sbar / c.l0;
-    add_at_last<VPL>(tbar_old, tp.ks, shfl3(ptb, tp.nl));
+    add_at_last<VPL>(tb2, tp.ks, shfl3(ptb, tp.nl));
     add_at_last<VPL>(A.d1, tp.ks, shfl3(pdb, tp.nl));
-    add_at_last<VPL>(iLbar_old, tp.ks, shfl(piLb, tp.nl));
+    add_at_last<VPL>(ib2, tp.ks, shfl(piLb, tp.nl));
     if (P.stretch_mode == 0) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
         if (tp.evalid[k]) {
           const f3 Fb = fbar[k] - next_of<VPL>(fbar, fb_next, k, tp.ks);
-          const float L = 1.0f / ec0.iL[k], eps = L / c.l0 - 1.0f, Ft = dot(Fb, ec0.t[k]);
+          const float L = 1.0f / eb0.iL[k], eps = L / c.l0 - 1.0f, Ft = dot(Fb, eb0.t[k]);
           G.gm[GM_STRETCH] += eps * Ft;
-          tbar_old[k] += (c.stretch * eps) * Fb;
-          iLbar_old[k] -= (c.stretch * Ft / c.l0) * L * L;
+          tb2[k] += (c.stretch * eps) * Fb;
+          ib2[k] -= (c.stretch * Ft / c.l0) * L * L;
         }
       }
     }
     f3 send = zero3<float>();
 #pragma unroll
     for (int k = 0; k < VPL; ++k)
-      if (tp.evalid[k]) scatter_edge<VPL>(A.x, send, k, tp.ks, normalize_adj<float>(ec0.t[k], ec0.iL[k], tbar_old[k], iLbar_old[k]));
+      if (tp.evalid[k]) scatter_edge<VPL>(A.x, send, k, tp.ks, normalize_adj<float>(eb0.t[k], eb0.iL[k], tb2[k], ib2[k]));
     A.x[0] += shfl3(send, tp.pl);
   }
 
@@ -341,10 +360,9 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
 #pragma unroll
     for (int k = 0; k < 6; ++k) { G.apbar[k] = 0.0f; G.acbar[k] = 0.0f; }
     for (int sub = P.n_sub - 1; sub >= 0; --sub) {
-      LaneState<VPL> s0;
-      load_state<VPL>(P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk, tp.base, P.NS, s0);
+      const float* s0blk = P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk;
       const int cflag = P.tape_flag ? (int)P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] : 1;
-      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0, A, G, acc_tape, cflag);
+      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, A, G, acc_tape, cflag);
     }
     if (P.g_actions && tp.lane < P.G) {
       float* gc = P.g_actions + (((size_t)t * P.B + env) * P.G + tp.lane) * 6;
