@@ -155,7 +155,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     const int per_adj = smem_layout(Pa, s->VPL, true);
     const int cap = 227 * 1024;
     if (per_adj > cap) { delete s; return fail(DLO_ERR_UNSUPPORTED, "shared memory per env exceeds 227 KB for this n_verts / n_proj_iters"); }
-    s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, (cap / 3) / std::max(per_fwd, 1)));   // three CTAs per SM
+    s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, (cap / 4) / std::max(per_fwd, 1)));   // four CTAs per SM
     s->wpb_adj = std::max(1, std::min(DLO_ADJ_WARPS, cap / std::max(per_adj, 1)));
     s->smem_fwd = per_fwd * s->wpb_fwd;
     s->smem_adj = per_adj * s->wpb_adj;

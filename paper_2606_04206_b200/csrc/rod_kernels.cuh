@@ -133,10 +133,20 @@ __device__ __forceinline__ void warp_setup(const KParams& P, int env, int lane, 
     const float* src = P.prim + ((size_t)env * P.K + k) * PRIM_NP;
     float* dst = sm.prim + k * PRIM_SM_STRIDE;
     for (int q = 0; q < PRIM_NP; ++q) dst[q] = src[q];
-    if (P.prim_type[k] == 3) {
+    const int ty = P.prim_type[k];
+    if (ty == 3) {
       M3<float> R = rodrigues<float>(mk3<float>(src[6], src[7], src[8]));
       for (int q = 0; q < 9; ++q) dst[6 + q] = R.m[q];
     }
+    // bounding sphere
+    dst[PRIM_BC] = src[0]; dst[PRIM_BC + 1] = src[1]; dst[PRIM_BC + 2] = src[2];
+    dst[PRIM_BR] = -1.0f;
+    if (ty == 1) {
+      const f3 a = mk3<float>(src[0], src[1], src[2]), b = mk3<float>(src[3], src[4], src[5]), mid = 0.5f * (a + b), hb = 0.5f * (b - a);
+      dst[PRIM_BC] = mid.x; dst[PRIM_BC + 1] = mid.y; dst[PRIM_BC + 2] = mid.z;
+      dst[PRIM_BR] = sqrt_(dot(hb, hb)) + src[6];
+    } else if (ty == 2) dst[PRIM_BR] = sqrt_(src[6] * src[6] + src[7] * src[7]);
+    else if (ty == 3) dst[PRIM_BR] = sqrt_(src[3] * src[3] + src[4] * src[4] + src[5] * src[5]);
   }
   for (int k = lane; k < P.G * P.M * 3; k += 32) sm.q[k] = P.qloc[(size_t)env * P.G * P.M * 3 + k];
   if (P.self_contact)
@@ -164,7 +174,7 @@ template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  write_tape: the state at
 // the start of every substep goes to P.tape (replay half of the reverse pass).
 template <int VPL>
-__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 3 : 2) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
+__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 4 : 2) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
   extern __shared__ __align__(16) float smem[];
   const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
   if (env >= P.B) return;

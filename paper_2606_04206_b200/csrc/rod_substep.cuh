@@ -66,6 +66,9 @@ __device__ __forceinline__ void publish_poses(const KParams& P, int env, int lan
     o[POSE_FA0] = A0.x; o[POSE_FA0 + 1] = A0.y; o[POSE_FA0 + 2] = A0.z; o[POSE_FB0] = B0.x; o[POSE_FB0 + 1] = B0.y; o[POSE_FB0 + 2] = B0.z;
     o[POSE_FA1] = A1.x; o[POSE_FA1 + 1] = A1.y; o[POSE_FA1 + 2] = A1.z; o[POSE_FB1] = B1.x; o[POSE_FB1 + 1] = B1.y; o[POSE_FB1 + 2] = B1.z;
     o[POSE_RF] = fg[2];
+    const f3 c0 = 0.5f * (A0 + B0), c1 = 0.5f * (A1 + B1);
+    o[POSE_FC0] = c0.x; o[POSE_FC0 + 1] = c0.y; o[POSE_FC0 + 2] = c0.z; o[POSE_FC1] = c1.x; o[POSE_FC1 + 1] = c1.y; o[POSE_FC1 + 2] = c1.z;
+    o[POSE_FRAD] = 0.5f * fabsf(len) + fg[2];
   }
   __syncwarp();
 }
@@ -319,16 +322,28 @@ struct CoupleOut { f3 v; unsigned active; };
 __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* __restrict__ prim_sm, const float* __restrict__ pose_sm,
                                                  f3 y, f3 v, float mu_r) {
   unsigned active = 0u;
+  // a body whose bounding sphere is farther than reach = r + eps_s |ln f_thresh| cannot pass the f > f_thresh test
+  const float reach = P.r - P.log_thresh_lo * (1.0f / P.inv_eps);
   for (int k = 0; k < P.K; ++k) {
+    const float* pk = prim_sm + k * PRIM_SM_STRIDE;
+    if (pk[PRIM_BR] >= 0.0f) {
+      const f3 dc = y - mk3<float>(pk[PRIM_BC], pk[PRIM_BC + 1], pk[PRIM_BC + 2]);
+      const float lim = pk[PRIM_BR] + reach;
+      if (dot(dc, dc) >= lim * lim) continue;
+    }
     float phi;
     f3 n;
-    if (!sdf_eval_pre<float>(P.prim_type[k], prim_sm + k * PRIM_SM_STRIDE, y, phi, n)) continue;
+    if (!sdf_eval_pre<float>(P.prim_type[k], pk, y, phi, n)) continue;
     if ((P.r - phi) * P.inv_eps < P.log_thresh_lo) continue;
     if (rigid_response<float>(v, zero3<float>(), n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << k;
   }
   for (int g = 0; g < P.G; ++g) {
     const float* o = pose_sm + g * POSE_STRIDE;
     for (int fk = 0; fk < 2; ++fk) {
+      const float* fc = o + (fk ? POSE_FC1 : POSE_FC0);
+      const f3 dc = y - mk3<float>(fc[0], fc[1], fc[2]);
+      const float lim = o[POSE_FRAD] + reach;
+      if (dot(dc, dc) >= lim * lim) continue;
       const float* A = o + (fk ? POSE_FA1 : POSE_FA0);
       const float* Bp = o + (fk ? POSE_FB1 : POSE_FB0);
       float Pc[7] = {A[0], A[1], A[2], Bp[0], Bp[1], Bp[2], o[POSE_RF]};

@@ -20,7 +20,9 @@ enum { MAT_M = 0, MAT_L0, MAT_STRETCH, MAT_ALPHA, MAT_GAMMA, MAT_SIGY, MAT_RC, M
 enum { ROW_X = 0, ROW_V = 3, ROW_D1 = 6, ROW_KB = 9, STATE_ROWS = 11 };
 enum { FLAG_NONFINITE = 1, FLAG_CAND_OVERFLOW = 2 };
 #define DLO_FULL 0xffffffffu
-enum { PRIM_NP = 10, PRIM_SM_STRIDE = 16 };   // boxes are expanded to centre(3), half(3), R(9) in shared memory
+// primitives in shared memory: [0..14] parameters (boxes expanded to centre(3), half(3), R(9)), [16..18] centre and [19]
+// radius of a bounding sphere (radius < 0: unbounded, e.g. a plane) used to cull vertices that are out of reach
+enum { PRIM_NP = 10, PRIM_SM_STRIDE = 20, PRIM_BC = 16, PRIM_BR = 19 };
 
 struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
@@ -48,7 +50,7 @@ struct KParams {
 };
 
 // per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
-enum { POSE_P0 = 0, POSE_R0 = 3, POSE_P1 = 12, POSE_R1 = 15, POSE_FA0 = 24, POSE_FB0 = 27, POSE_FA1 = 30, POSE_FB1 = 33, POSE_RF = 36, POSE_STRIDE = 40 };
+enum { POSE_P0 = 0, POSE_R0 = 3, POSE_P1 = 12, POSE_R1 = 15, POSE_FA0 = 24, POSE_FB0 = 27, POSE_FA1 = 30, POSE_FB1 = 33, POSE_RF = 36, POSE_FC0 = 37, POSE_FC1 = 40, POSE_FRAD = 43, POSE_STRIDE = 44 };   // FC*: finger mid points, FRAD: bounding radius
 
 __device__ __forceinline__ float shfl(float v, int src) { return __shfl_sync(DLO_FULL, v, src); }
 __device__ __forceinline__ f3 shfl3(const f3& v, int src) { return mk3<float>(shfl(v.x, src), shfl(v.y, src), shfl(v.z, src)); }
