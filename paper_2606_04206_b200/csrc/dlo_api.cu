@@ -155,7 +155,17 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     const int per_adj = smem_layout(Pa, s->VPL, true);
     const int cap = 227 * 1024;
     if (per_adj > cap) { delete s; return fail(DLO_ERR_UNSUPPORTED, "shared memory per env exceeds 227 KB for this n_verts / n_proj_iters"); }
-    s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, (cap / 4) / std::max(per_fwd, 1)));   // four CTAs per SM
+    // forward: two CTAs per SM; choose the CTA size whose slots (2 * n_SM * warps) split the batch into whole waves
+    // (4096 envs on 148 SMs: 7 warps -> 1.98 waves, where 8 warps would leave the second wave 27 % empty)
+    int n_sm = 148;
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+    const int max_c = std::max(1, std::min(DLO_FWD_WARPS, (cap / 2) / std::max(per_fwd, 1)));
+    double best = 1e30;
+    s->wpb_fwd = max_c;
+    for (int cw = std::min(4, max_c); cw <= max_c; ++cw) {
+      const double slots = 2.0 * n_sm * cw, waves = ceil(P.B / slots), cost = waves * sqrt((double)cw);
+      if (cost < best - 1e-9) { best = cost; s->wpb_fwd = cw; }
+    }
     s->wpb_adj = std::max(1, std::min(DLO_ADJ_WARPS, cap / std::max(per_adj, 1)));
     s->smem_fwd = per_fwd * s->wpb_fwd;
     s->smem_adj = per_adj * s->wpb_adj;

@@ -6,9 +6,9 @@
 namespace dlo {
 
 // warps (= envs) per CTA: the CTA's warps walk the kernel in lockstep (phase_sync), so more warps per CTA share each
-// instruction-cache fill.  Forward: 3 CTAs of 4 warps per SM at 168 registers (measured faster than 2 x 6 and 1 x 12); adjoint: 1 CTA of 8 warps at 255.
+// instruction-cache fill.  Forward: 2 CTAs of 4..8 warps per SM at <= 128 registers; the host picks the count that fills whole waves; adjoint: 1 CTA of 8 warps at 255.
 // (upper bounds: the host lowers them when the per-warp shared memory of a large rope would not fit)
-#define DLO_FWD_WARPS 4
+#define DLO_FWD_WARPS 8
 #define DLO_ADJ_WARPS 8
 
 // ---------------------------------------------------------------------------------------------------------
@@ -174,7 +174,7 @@ template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  write_tape: the state at
 // the start of every substep goes to P.tape (replay half of the reverse pass).
 template <int VPL>
-__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 4 : 2) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
+__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
   extern __shared__ __align__(16) float smem[];
   const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
   if (env >= P.B) return;
