@@ -389,7 +389,6 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   }
   bending_forces<VPL>(tp, s, ec, c.alpha / c.l0, f);
 
-  phase_sync(sm);
   // -- A3 velocity (symplectic Euler L97, implicit viscous damping R-7), A4 predict
   const float idamp = 1.0f / (1.0f + c.gamma * h), hm = h * c.inv_m;
 #pragma unroll
@@ -555,7 +554,6 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     }
   }
 
-  phase_sync(sm);
   // -- A6 reconcile v with the projected positions (R-11) + self-contact friction
   f3 vel[VPL];
 #pragma unroll
@@ -588,7 +586,6 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     R.v4[k] = vel[k];
   }
 
-  phase_sync(sm);
   // -- A8 commit
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
