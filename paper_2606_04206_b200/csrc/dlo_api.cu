@@ -116,7 +116,7 @@ size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
   n += 2 * B * blk;                                                            // state, state0
   if (stride > 0 && horizon > 0) {
     n += ((size_t)horizon / stride + 1) * B * blk;                             // checkpoints
-    n += (size_t)(stride < horizon ? stride : horizon) * P.n_sub * B * blk;    // per-substep tape of one segment
+    n += ((size_t)(stride < horizon ? stride : horizon) * P.n_sub + 1) * B * tape_rows(P.N_C) * P.NS * sizeof(float);   // tape of one segment
     n += B * blk;                                                              // running adjoint
     if (P.self_contact) n += B * (size_t)P.N_C * 3 * 33 * vpl_for(P.N) * 4;    // self-contact correction tape
   }
@@ -283,30 +283,29 @@ dlo_status dlo_set_actions(dlo_sim* s, const float* actions, int32_t horizon) {
 
 }  // extern "C"
 
-template <int VPL> static cudaError_t launch_forward_t(dlo_sim* s, int t0, int t1, int stride, int write_tape) {
-  static bool attr_done = false;
-  if (!attr_done || s->smem_fwd > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(k_forward<VPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fwd > 48 * 1024 ? s->smem_fwd : 48 * 1024);
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
-  const int grid = (s->P.B + s->wpb_fwd - 1) / s->wpb_fwd;
-  k_forward<VPL><<<grid, s->wpb_fwd * 32, s->smem_fwd, s->stream>>>(s->P, t0, t1, stride, write_tape);
+template <int VPL, bool TAPE> static cudaError_t launch_forward_t(dlo_sim* s, const KParams& P, int t0, int t1, int stride) {
+  cudaError_t e = cudaFuncSetAttribute(k_forward<VPL, TAPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fwd > 48 * 1024 ? s->smem_fwd : 48 * 1024);
+  if (e != cudaSuccess) return e;
+  const int grid = (P.B + s->wpb_fwd - 1) / s->wpb_fwd;
+  k_forward<VPL, TAPE><<<grid, s->wpb_fwd * 32, s->smem_fwd, s->stream>>>(P, t0, t1, stride);
   s->launches += 1;
   return cudaGetLastError();
 }
-static cudaError_t launch_forward(dlo_sim* s, int t0, int t1, int stride, int write_tape) {
-  smem_layout(s->P, s->VPL, false);
+// forward (tape = false) or replay of a segment with tape records (tape = true); P carries the buffers to use
+static cudaError_t launch_forward(dlo_sim* s, KParams P, int t0, int t1, int stride, bool tape) {
+  smem_layout(P, s->VPL, false);
+#define DLO_FWD_CASE(V) return tape ? launch_forward_t<V, true>(s, P, t0, t1, stride) : launch_forward_t<V, false>(s, P, t0, t1, stride)
   switch (s->VPL) {
 #ifdef DLO_VPL_ONLY   /* development builds: one instantiation only */
-    default: return launch_forward_t<DLO_VPL_ONLY>(s, t0, t1, stride, write_tape);
+    default: DLO_FWD_CASE(DLO_VPL_ONLY);
 #else
-    case 2: return launch_forward_t<2>(s, t0, t1, stride, write_tape);
-    case 4: return launch_forward_t<4>(s, t0, t1, stride, write_tape);
-    case 6: return launch_forward_t<6>(s, t0, t1, stride, write_tape);
-    default: return launch_forward_t<8>(s, t0, t1, stride, write_tape);
+    case 2: DLO_FWD_CASE(2);
+    case 4: DLO_FWD_CASE(4);
+    case 6: DLO_FWD_CASE(6);
+    default: DLO_FWD_CASE(8);
 #endif
   }
+#undef DLO_FWD_CASE
 }
 
 extern "C" {
@@ -332,7 +331,7 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     s->P.ckpt = s->ckpt;
     CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
   }
-  if (horizon > 0) CU(launch_forward(s, 0, horizon, stride, 0));
+  if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;
 }

@@ -27,12 +27,12 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
   if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
   const int H = s->H_done, stride = s->stride, B = s->P.B;
-  const size_t blk = s->blk, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub;
+  const size_t blk = s->blk, rec = (size_t)tape_rows(s->P.N_C) * s->P.NS, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub + 1;
   if (seg > s->tape_blocks) {
     CU(cudaStreamSynchronize(s->stream));
     if (s->tape) cudaFree(s->tape);
     s->tape = nullptr; s->tape_blocks = 0;
-    CU(dalloc(&s->tape, seg * B * blk));
+    CU(dalloc(&s->tape, seg * B * rec));
     if (s->tape_flag) cudaFree(s->tape_flag);
     s->tape_flag = nullptr;
     CU(dalloc(&s->tape_flag, seg * B));
@@ -56,15 +56,8 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
     // replay the segment from its checkpoint, leaving the state at the start of every substep on the tape
     KParams Pf = s->P;
-    smem_layout(Pf, s->VPL, false);
     Pf.state = s->replay; Pf.tape = s->tape; Pf.tape_flag = s->tape_flag;
-    {
-      dlo_sim tmp = *s;   // launch through the same path as the forward, on the replay buffer
-      tmp.P = Pf;
-      cudaError_t e = launch_forward(&tmp, t0, t1, 0, 1);
-      s->launches = tmp.launches;
-      if (e != cudaSuccess) return fail(DLO_ERR_CUDA, std::string("replay launch: ") + cudaGetErrorString(e));
-    }
+    CU(launch_forward(s, Pf, t0, t1, 0, true));
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
     Pa.tape = s->tape; Pa.tape_flag = s->tape_flag; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;

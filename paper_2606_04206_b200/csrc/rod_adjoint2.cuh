@@ -28,7 +28,7 @@ __device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float w
 template <int VPL>
 __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                                 const float ap[6], const float ac[6], int sub, const float* __restrict__ s0blk,
-                                                LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag) {
+                                                const float* __restrict__ s1blk, LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag) {
   const float h = P.h, inv_h = P.inv_h;
   // ---- forward recompute with recording.  The start state is read from the tape twice (here and again for the
   // reverse of A2) rather than held in ~70 registers across the projection loop, the hottest part of the kernel.
@@ -43,9 +43,45 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.G > 0) {
     for (int k = tp.lane; k < P.G * 24; k += 32) sm.posebar[k] = 0.0f;
   }
-  ContactCache<VPL> cc;
-  cc.reset(contact_flag ? -1.0f : 1.0e30f);   // the replay saw no self-contact correction in this substep: skip it outright
-  substep<VPL, true>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc);
+  if (contact_flag) {
+    // the substep applied a self-contact correction: recompute it with recording (candidate list, depth sums, corrections)
+    ContactCache<VPL> cc;
+    cc.reset(-1.0f);
+    substep<VPL, 1>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc);
+  } else {
+    // common case: everything the reverse needs is on the tape record written by the replay
+    load_rows3<VPL>(s0blk + (size_t)TAPE_XP * P.NS, tp.base, P.NS, R.xp);
+    load_rows3<VPL>(s0blk + (size_t)TAPE_DX * P.NS, tp.base, P.NS, R.dx);
+    load_rows3<VPL>(s0blk + (size_t)TAPE_V3 * P.NS, tp.base, P.NS, R.v3);
+    load_row<VPL>(s0blk + (size_t)TAPE_S * P.NS, tp.base, P.NS, R.S);
+    float am[VPL];
+    load_row<VPL>(s0blk + (size_t)TAPE_ACT * P.NS, tp.base, P.NS, am);
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      R.active[k] = __float_as_uint(am[k]);
+      R.v1[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v3[k], -inv_h, R.dx[k]) : R.v3[k];   // v^3 = v^1 + dx/h without friction
+      R.t_old[k] = ec0.t[k];
+    }
+    R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
+    for (int it = 0; it < P.N_C; ++it) {
+      float lamv[VPL];
+      load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it) * P.NS, tp.base, P.NS, lamv);
+      float lam3 = 0.0f;
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) {
+        sm.lam[(it * VPL + k) * 32 + tp.lane] = lamv[k];
+        if (P.odd_ring && k == tp.ks && tp.base + k == P.E - 1) lam3 = lamv[k];
+      }
+      if (P.odd_ring) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
+    }
+    // state at the end of the substep = start state of the next record (positions and directors are all that is used)
+    load_rows3<VPL>(s1blk + (size_t)ROW_X * P.NS, tp.base, P.NS, s.x);
+    load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
+    edge_refresh<VPL>(tp, s, ec);
+    edge_prev_refresh<VPL>(tp, s, ec);
+#pragma unroll
+    for (int q = 0; q < SUBSTEP_SYNCS; ++q) phase_sync(sm);
+  }
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
 
   f3 tbar_old[VPL], tbar_new[VPL];
@@ -252,7 +288,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (c.kin[k] == KIN_FREE) {
       A.v[k] = idamp * v1bar[k];
       fbar[k] = (hm * idamp) * v1bar[k];
-      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], inv_h * (R.xp[k] - s0b.x[k]));   // v^1 = (x^p - x)/h
+      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], R.v1[k]);
     } else if (c.kin[k] >= KIN_GRASP0) {
       const f3 tb = inv_h * v1bar[k];
       grasp_target_adj(P, sm, c.kin[k], tb);
@@ -360,9 +396,11 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
 #pragma unroll
     for (int k = 0; k < 6; ++k) { G.apbar[k] = 0.0f; G.acbar[k] = 0.0f; }
     for (int sub = P.n_sub - 1; sub >= 0; --sub) {
-      const float* s0blk = P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk;
+      const size_t rec = (size_t)tape_rows(P.N_C) * P.NS, idx = (size_t)(t - t0) * P.n_sub + sub;
+      const float* s0blk = P.tape + (idx * P.B + env) * rec;
+      const float* s1blk = P.tape + ((idx + 1) * P.B + env) * rec;
       const int cflag = P.tape_flag ? (int)P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] : 1;
-      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, A, G, acc_tape, cflag);
+      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, s1blk, A, G, acc_tape, cflag);
     }
     if (P.g_actions && tp.lane < P.G) {
       float* gc = P.g_actions + (((size_t)t * P.B + env) * P.G + tp.lane) * 6;

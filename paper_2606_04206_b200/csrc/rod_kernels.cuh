@@ -173,8 +173,37 @@ template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<
 // Persistent forward segment: steps t0..t1-1 of every env, one warp per env, state in registers throughout.
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  write_tape: the state at
 // the start of every substep goes to P.tape (replay half of the reverse pass).
-template <int VPL>
-__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride, int write_tape) {
+// rows of one tape record (per substep and env), each NS floats: the state at the start of the substep, then what the
+// reverse pass would otherwise have to recompute: predicted positions, final corrections, the velocity before the rigid
+// coupling (differencing positions would cost too many digits), Eq.10 multiplier sums, the
+// mask of rigid bodies that responded, and the multipliers of every iteration
+enum { TAPE_XP = STATE_ROWS, TAPE_DX = TAPE_XP + 3, TAPE_V3 = TAPE_DX + 3, TAPE_S = TAPE_V3 + 3, TAPE_ACT = TAPE_S + 1, TAPE_LAM = TAPE_ACT + 1 };
+__host__ __device__ inline int tape_rows(int N_C) { return TAPE_LAM + N_C; }
+
+template <int VPL> __device__ __forceinline__ void store_rows3(float* __restrict__ rows, int base, int NS, const f3 a[VPL]) {
+  float r[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].x;
+  store_row<VPL>(rows, base, NS, r);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].y;
+  store_row<VPL>(rows + NS, base, NS, r);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].z;
+  store_row<VPL>(rows + 2 * NS, base, NS, r);
+}
+template <int VPL> __device__ __forceinline__ void load_rows3(const float* __restrict__ rows, int base, int NS, f3 a[VPL]) {
+  float rx[VPL], ry[VPL], rz[VPL];
+  load_row<VPL>(rows, base, NS, rx); load_row<VPL>(rows + NS, base, NS, ry); load_row<VPL>(rows + 2 * NS, base, NS, rz);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) a[k] = mk3<float>(rx[k], ry[k], rz[k]);
+}
+
+// Persistent forward segment: steps t0..t1-1 of every env, one warp per env, state in registers throughout.
+// stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  TAPE = true is the replay half of
+// the reverse pass: a tape record per substep goes to P.tape, and the segment's final state to record [n_substeps].
+template <int VPL, bool TAPE>
+__global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride) {
   extern __shared__ __align__(16) float smem[];
   const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
   if (env >= P.B) return;
@@ -186,7 +215,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
   EnvConst<VPL> c;
   load_env<VPL>(P, env, tp, c);
   warp_setup<VPL>(P, env, tp.lane, sm);
-  const size_t blk = (size_t)STATE_ROWS * P.NS;
+  const size_t blk = (size_t)STATE_ROWS * P.NS, rec = (size_t)tape_rows(P.N_C) * P.NS;
   LaneState<VPL> s;
   load_state<VPL>(P.state + (size_t)env * blk, tp.base, P.NS, s);
   EdgeCache<VPL> ec;
@@ -199,12 +228,27 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
   for (int t = t0; t < t1; ++t) {
     if (P.G > 0) load_actions(P, env, tp.lane, t, ap, ac);
     for (int sub = 0; sub < P.n_sub; ++sub) {
-      if (write_tape) store_state<VPL>(P.tape + ((size_t)((t - t0) * P.n_sub + sub) * P.B + env) * blk, tp.base, P.NS, s);
-      substep<VPL, false>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
-      if (write_tape && P.tape_flag && tp.lane == 0) P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] = (uint8_t)R.any_pen;
+      if (TAPE) {
+        const size_t idx = (size_t)(t - t0) * P.n_sub + sub;
+        float* tb = P.tape + (idx * P.B + env) * rec;
+        store_state<VPL>(tb, tp.base, P.NS, s);
+        substep<VPL, 2>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc, tb + (size_t)TAPE_LAM * P.NS);
+        store_rows3<VPL>(tb + (size_t)TAPE_XP * P.NS, tp.base, P.NS, R.xp);
+        store_rows3<VPL>(tb + (size_t)TAPE_DX * P.NS, tp.base, P.NS, R.dx);
+        store_rows3<VPL>(tb + (size_t)TAPE_V3 * P.NS, tp.base, P.NS, R.v3);
+        store_row<VPL>(tb + (size_t)TAPE_S * P.NS, tp.base, P.NS, R.S);
+        float am[VPL];
+#pragma unroll
+        for (int k = 0; k < VPL; ++k) am[k] = __uint_as_float(R.active[k]);
+        store_row<VPL>(tb + (size_t)TAPE_ACT * P.NS, tp.base, P.NS, am);
+        if (tp.lane == 0) P.tape_flag[idx * P.B + env] = (uint8_t)R.any_pen;
+      } else {
+        substep<VPL, 0>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
+      }
     }
     if (stride > 0 && (t + 1) % stride == 0) store_state<VPL>(P.ckpt + ((size_t)((t + 1) / stride) * P.B + env) * blk, tp.base, P.NS, s);
   }
+  if (TAPE) store_state<VPL>(P.tape + ((size_t)(t1 - t0) * P.n_sub * P.B + env) * rec, tp.base, P.NS, s);
   store_state<VPL>(P.state + (size_t)env * blk, tp.base, P.NS, s);
   const bool ok = state_finite<VPL>(s);
   if (__any_sync(DLO_FULL, !ok) && tp.lane == 0) atomicOr(P.flags + env, FLAG_NONFINITE);

@@ -363,10 +363,15 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
 // ---------------------------------------------------------------------------------------------------------
 // One substep.  On entry `ec` holds the edge geometry of s.x (tangents, inverse lengths, previous lane's last
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
-template <int VPL, bool REC>
+// number of phase_sync() calls inside substep(): a warp that skips the recompute must still take part in them
+enum { SUBSTEP_SYNCS = 4 };
+// MODE 0: plain forward.  MODE 1 (REC): recompute inside the adjoint kernel, multipliers -> shared memory, contact
+// corrections -> acc_tape.  MODE 2 (TAPE): replay of a segment, multipliers -> the global tape rows `lam_rows` [N_C][NS].
+template <int VPL, int MODE>
 __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                         const float ap[6], const float ac[6], int sub, LaneState<VPL>& s, EdgeCache<VPL>& ec,
-                                        SubRec<VPL>& R, float* acc_tape, ContactCache<VPL>& cc) {
+                                        SubRec<VPL>& R, float* acc_tape, ContactCache<VPL>& cc, float* lam_rows = nullptr) {
+  constexpr bool REC = MODE == 1;
   const float h = P.h, inv_h = P.inv_h;
   // -- A1 bodies
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);
@@ -460,6 +465,9 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
   for (int it = 0; it < P.N_C; ++it) {
+    float lamv[VPL];
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) lamv[k] = 0.0f;
     if (P.stretch_mode == 1) {
       // red: even slots, both end points local
 #pragma unroll
@@ -473,6 +481,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
         R.dx[k + 1] = axpy(R.dx[k + 1], -lam * c.w[k + 1], t);
         if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
+        lamv[k] = lam;
       }
       // black: odd slots; the lane's last slot crosses to slot 0 of the next lane
       {
@@ -493,6 +502,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
           if (rem) { if (on) back = (lam * wn) * t; }
           else if (k + 1 < VPL) R.dx[k + 1] = axpy(R.dx[k + 1], -lam * wn, t);
           if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
+          lamv[k] = lam;
         }
         R.dx[0] -= shfl3(back, tp.pl);
       }
@@ -512,12 +522,14 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
             R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
             back = (lam * c.wr) * t;
             lam3 = lam;
+            lamv[k] = lam;   // the closing edge's slot is idle in the red sweep
           }
         }
         R.dx[0] -= shfl3(back, tp.pl);
         if (REC) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
       }
     }
+    if (MODE == 2 && lam_rows) store_row<VPL>(lam_rows + (size_t)it * P.NS, tp.base, P.NS, lamv);
     bool sweep = false;
     if (P.self_contact) {
       float m2 = 0.0f;

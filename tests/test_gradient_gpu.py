@@ -100,7 +100,9 @@ def test_gradient_independent_of_stride(dlo):
         sim.close()
     for o in outs[1:]:
         for k in ("g_actions", "g_x0", "g_v0", "g_material"):
-            assert np.allclose(o[k], outs[0][k], rtol=1e-4, atol=1e-7 * np.abs(outs[0][k]).max()), k
+            # identical trajectory, different grouping of the fp32 sums (per-segment accumulation, shared-memory atomics
+            # for the gripper poses): agreement to rounding level, relative to the largest entry
+            assert np.abs(o[k] - outs[0][k]).max() <= 5e-5 * np.abs(outs[0][k]).max(), k
 
 
 # Kinked cases: Eq.11 drives every active hinge onto its yield surface
