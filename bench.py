@@ -28,9 +28,10 @@ from workloads.configs import make_problem, loss_and_seed, FULL_SIZES  # noqa: E
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"
-# Algorithmic fp32 flops per env-step of config 5 (5 substeps, N=128, N_C=10), DESIGN.md section 7:
-# forward 1.2e6; forward+backward = forward + replay + adjoint(2.5x) = 4.5x.
-FLOPS_PER_ENV_STEP = {"fwd": 1.2e6, "fwdbwd": 5.4e6}
+# Algorithmic fp32 flops per env-step of config 5 (5 substeps, N=128, N_C=10, 4 primitives + 4 finger capsules), counted
+# in DESIGN.md section 7 (FADD/FMUL = 1, FFMA = 2): forward 0.10 Mflop per substep = 0.5 Mflop per env-step; the reverse of a
+# substep 0.17 Mflop; forward+backward = forward + replay + reverse = 0.5 + 0.5 + 0.85 = 1.85 Mflop per env-step.
+FLOPS_PER_ENV_STEP = {"fwd": 0.5e6, "fwdbwd": 1.85e6}
 # fp32 ALU peak derived in DESIGN.md section 7: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
