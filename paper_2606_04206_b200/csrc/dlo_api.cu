@@ -67,7 +67,6 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
     P.sm_blk = take(4 * 32);
   }
   if (adjoint) {
-    P.sm_lam = take((P.N_C * VPL + P.N_C) * 32);
     P.sm_posebar = take(P.G * 24);
     if (P.self_contact) { P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP); }
   }

@@ -47,7 +47,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     // the substep applied a self-contact correction: recompute it with recording (candidate list, depth sums, corrections)
     ContactCache<VPL> cc;
     cc.reset(-1.0f);
-    substep<VPL, 1>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc);
+    substep<VPL, 1>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc, const_cast<float*>(s0blk) + (size_t)TAPE_LAM * P.NS);
   } else {
     // common case: everything the reverse needs is on the tape record written by the replay
     load_rows3<VPL>(s0blk + (size_t)TAPE_XP * P.NS, tp.base, P.NS, R.xp);
@@ -63,17 +63,6 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       R.t_old[k] = ec0.t[k];
     }
     R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
-    for (int it = 0; it < P.N_C; ++it) {
-      float lamv[VPL];
-      load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it) * P.NS, tp.base, P.NS, lamv);
-      float lam3 = 0.0f;
-#pragma unroll
-      for (int k = 0; k < VPL; ++k) {
-        sm.lam[(it * VPL + k) * 32 + tp.lane] = lamv[k];
-        if (P.odd_ring && k == tp.ks && tp.base + k == P.E - 1) lam3 = lamv[k];
-      }
-      if (P.odd_ring) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
-    }
     // state at the end of the substep = start state of the next record (positions and directors are all that is used)
     load_rows3<VPL>(s1blk + (size_t)ROW_X * P.NS, tp.base, P.NS, s.x);
     load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
@@ -208,6 +197,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   const float atil = c.stretch * inv_h * inv_h;
   float atilbar = 0.0f;
   for (int it = P.N_C - 1; it >= 0; --it) {
+    float lamv[VPL];   // multipliers of this iteration, one per owned edge (the odd ring's closing edge sits in its idle red slot)
+    load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it) * P.NS, tp.base, P.NS, lamv);
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
@@ -235,7 +226,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 #pragma unroll
         for (int k = 0; k < VPL; k += 2) {
           if (k == tp.ks && tp.base + k == P.E - 1 && c.w[k] + c.wr > 0.0f)
-            edge_reverse(epred[k], sm.lam[(P.N_C * VPL + it) * 32 + tp.lane], c.w[k], c.wr, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
+            edge_reverse(epred[k], lamv[k], c.w[k], c.wr, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
         }
         R.dx[0] += shfl3(dxr - dxr0, tp.pl);
         dxb[0] += shfl3(gr - gr0, tp.pl);
@@ -249,7 +240,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
           const bool on = tp.evalid[k] && (k <= tp.ks);
           const float wn = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
           if (on && c.w[k] + wn > 0.0f) {
-            const float lam = sm.lam[(it * VPL + k) * 32 + tp.lane];
+            const float lam = lamv[k];
             if (rem) edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
             else edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], R.dx[k + 1 < VPL ? k + 1 : k], R.S[k], dxb[k], dxb[k + 1 < VPL ? k + 1 : k], Sb[k], atilbar, epb[k]);
           }
@@ -261,7 +252,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       for (int k = 0; k < VPL; k += 2) {   // red
         const bool on = (k + 1 < tp.nv) && tp.evalid[k];
         if (on && c.w[k] + c.w[k + 1] > 0.0f)
-          edge_reverse(epred[k], sm.lam[(it * VPL + k) * 32 + tp.lane], c.w[k], c.w[k + 1], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
+          edge_reverse(epred[k], lamv[k], c.w[k], c.w[k + 1], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
       }
     }
   }

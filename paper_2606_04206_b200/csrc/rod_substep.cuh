@@ -365,8 +365,8 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
 // number of phase_sync() calls inside substep(): a warp that skips the recompute must still take part in them
 enum { SUBSTEP_SYNCS = 4 };
-// MODE 0: plain forward.  MODE 1 (REC): recompute inside the adjoint kernel, multipliers -> shared memory, contact
-// corrections -> acc_tape.  MODE 2 (TAPE): replay of a segment, multipliers -> the global tape rows `lam_rows` [N_C][NS].
+// MODE 0: plain forward.  MODE 1 (REC): recompute inside the adjoint kernel (contact corrections -> acc_tape).
+// MODE 2 (TAPE): replay of a segment.  In both, the Eq.10 multipliers go to the tape rows `lam_rows` [N_C][NS].
 template <int VPL, int MODE>
 __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                         const float ap[6], const float ac[6], int sub, LaneState<VPL>& s, EdgeCache<VPL>& ec,
@@ -480,7 +480,6 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         R.S[k] += lam;
         R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
         R.dx[k + 1] = axpy(R.dx[k + 1], -lam * c.w[k + 1], t);
-        if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
         lamv[k] = lam;
       }
       // black: odd slots; the lane's last slot crosses to slot 0 of the next lane
@@ -501,8 +500,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
           R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
           if (rem) { if (on) back = (lam * wn) * t; }
           else if (k + 1 < VPL) R.dx[k + 1] = axpy(R.dx[k + 1], -lam * wn, t);
-          if (REC) sm.lam[(it * VPL + k) * 32 + tp.lane] = lam;
-          lamv[k] = lam;
+            lamv[k] = lam;
         }
         R.dx[0] -= shfl3(back, tp.pl);
       }
@@ -526,10 +524,10 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
           }
         }
         R.dx[0] -= shfl3(back, tp.pl);
-        if (REC) sm.lam[(P.N_C * VPL + it) * 32 + tp.lane] = lam3;
+        (void)lam3;
       }
     }
-    if (MODE == 2 && lam_rows) store_row<VPL>(lam_rows + (size_t)it * P.NS, tp.base, P.NS, lamv);
+    if (MODE >= 1 && lam_rows) store_row<VPL>(lam_rows + (size_t)it * P.NS, tp.base, P.NS, lamv);
     bool sweep = false;
     if (P.self_contact) {
       float m2 = 0.0f;
