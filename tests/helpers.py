@@ -30,3 +30,24 @@ def rope_problem(x0, v0=None, *, ring=False, dt=1e-3, horizon=10, stride=0, mate
 def aos(a):
     """[B][3][N] -> [B][N][3]"""
     return np.asarray(a).transpose(0, 2, 1)
+
+
+def figure_eight_problem(N=32, gap=0.0062, B=2, horizon=30, stride=7, seed=0):
+    """An open rope laid as a figure eight whose two strands cross once, `gap` apart vertically, and move towards each
+    other slowly: one gentle self-contact (Eq.13) with sliding friction, no gravity.  Used to check the self-contact
+    path and its adjoint on a well-conditioned case."""
+    from workloads.configs import _resample_polyline
+    rng = np.random.default_rng(seed)
+    t = np.linspace(-0.3 * np.pi, 1.3 * np.pi, 2000)
+    curve = np.stack([0.04 * np.sin(2 * t), 0.04 * np.sin(t), 0.5 * gap * np.cos(t)], 1)
+    pts = _resample_polyline(curve, N)
+    x = pts[None].repeat(B, 0) + rng.normal(0, 5e-5, (B, N, 3))
+    v = np.zeros_like(x)
+    v[..., 2] = -15.0 * x[..., 2]
+    v[..., 0] = 0.05 * np.sign(x[..., 2])
+    l0 = np.linalg.norm(np.diff(pts, axis=0), axis=1).mean()
+    P = rope_problem(x, v, dt=1e-3, horizon=horizon, stride=stride, enable_self_contact=1, gravity=(0.0, 0.0, 0.0),
+                     material=dict(stretch=1e-6, alpha=2e-4, gamma=0.05, mu_s=0.4, l0=l0))
+    P["loss"] = dict(kind="polyline", target=np.zeros((B, 3, N)))
+    P["grad_wrt"] = ()
+    return P

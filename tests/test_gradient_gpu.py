@@ -80,6 +80,23 @@ def test_gradient_parity(dlo, orc, name, kw, H, stride, keys, over):
     check(name, got, ref, keys)
 
 
+def test_self_contact_crossing_gradient(dlo, orc):
+    """one real Eq.13 contact with friction (figure eight), well conditioned: forward and every gradient at the plain bars"""
+    from helpers import figure_eight_problem
+    from parity import POS_TOL, position_error
+    for H in (16, 30):
+        P = figure_eight_problem(horizon=H, stride=7)
+        free = dict(P, config=dict(P["config"], enable_self_contact=0))
+        a, b = orc.OracleSim(P).rollout(H, 0)["x"], orc.OracleSim(free).rollout(H, 0)["x"]
+        assert np.abs(a - b).max() > 1e-4, "the contact must actually engage"
+        got, ref = both_gradients(dlo, orc, P, H, 7)
+        check("figure eight H=%d" % H, got, ref, ("g_x0", "g_v0", "g_material"))
+        sim = dlo.DloSim(P)
+        x = sim.rollout(H, 0).state()["x"]
+        sim.close()
+        assert position_error(P, x, a).max() <= POS_TOL
+
+
 def test_stretch_energy_mode_gradient(dlo, orc):
     P = make_problem(1, n_verts=16, horizon=30, stride=10)
     P["config"]["stretch_mode"] = 0
