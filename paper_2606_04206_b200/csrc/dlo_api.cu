@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <string>
 #include <vector>
@@ -158,13 +159,18 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     // (4096 envs on 148 SMs: 7 warps -> 1.98 waves, where 8 warps would leave the second wave 27 % empty)
     int n_sm = 148;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
-    const int max_c = std::max(1, std::min(DLO_FWD_WARPS, (cap / 2) / std::max(per_fwd, 1)));
+    // CTA shape: c warps per CTA, as many CTAs per SM as 16 warps (128 registers) and shared memory allow.  Cost model
+    // fitted to a sweep on config 5: time ~ waves * sqrt(warps per SM), larger CTAs slightly
+    // better at equal occupancy (more warps share each instruction-cache fill).
     double best = 1e30;
-    s->wpb_fwd = max_c;
-    for (int cw = std::min(4, max_c); cw <= max_c; ++cw) {
-      const double slots = 2.0 * n_sm * cw, waves = ceil(P.B / slots), cost = waves * sqrt((double)cw);
+    s->wpb_fwd = 1;
+    for (int cw = 1; cw <= DLO_FWD_WARPS; ++cw) {
+      const int k = std::min(16 / cw, cap / std::max(cw * per_fwd, 1));
+      if (k < 1) continue;
+      const double slots = (double)k * n_sm * cw, waves = ceil(P.B / slots), cost = waves * sqrt((double)(k * cw)) * (1.0 - 0.01 * cw);
       if (cost < best - 1e-9) { best = cost; s->wpb_fwd = cw; }
     }
+    if (const char* ov = getenv("DLO_FWD_WARPS")) s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, atoi(ov)));   // tuning override
     s->wpb_adj = std::max(1, std::min(DLO_ADJ_WARPS, cap / std::max(per_adj, 1)));
     s->smem_fwd = per_fwd * s->wpb_fwd;
     s->smem_adj = per_adj * s->wpb_adj;
