@@ -172,6 +172,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     }
     if (const char* ov = getenv("DLO_FWD_WARPS")) s->wpb_fwd = std::max(1, std::min(DLO_FWD_WARPS, atoi(ov)));   // tuning override
     s->wpb_adj = std::max(1, std::min(DLO_ADJ_WARPS, cap / std::max(per_adj, 1)));
+    if (const char* ov = getenv("DLO_ADJ_WARPS")) s->wpb_adj = std::max(1, std::min(s->wpb_adj, atoi(ov)));   // tuning override
     s->smem_fwd = per_fwd * s->wpb_fwd;
     s->smem_adj = per_adj * s->wpb_adj;
   }
