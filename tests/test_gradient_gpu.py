@@ -157,3 +157,28 @@ def test_gradient_parity_at_kinks(dlo, orc, name, kw, H, stride, keys):
         print(summarize("%s %s gpu" % (name, k), err), "|", summarize("oracle spread", spread[k]), "| outside: %d" % (~ok).sum())
         assert np.median(err) <= GRAD_TOL, (name, k, np.median(err))
         assert (~ok).sum() <= len(err) // 4, (name, k, err, spread[k])
+
+
+@pytest.mark.parametrize("N,ring", [(3, False), (4, True), (5, True), (256, False), (255, True)],
+                         ids=["N=3 open", "N=4 ring", "N=5 odd ring", "N=256 open", "N=255 odd ring"])
+def test_gradient_extreme_sizes(dlo, orc, N, ring):
+    """smallest and largest ropes (every lanes-per-env layout, ring wrap through lane 0, third colour of odd rings)"""
+    from helpers import rope_problem
+    rng = np.random.default_rng(9)
+    B, H = 2, 8
+    if ring:
+        th = np.linspace(0, 2 * np.pi, N, endpoint=False)
+        x = np.stack([0.1 * np.cos(th), 0.1 * np.sin(th), 0.02 * np.sin(2 * th)], 1)
+    else:
+        x = np.stack([np.arange(N) * (0.5 / (N - 1)), np.zeros(N), np.zeros(N)], 1)
+    x = x[None].repeat(B, 0) + rng.normal(0, 2e-4, (B, N, 3))
+    P = rope_problem(x, rng.normal(0, 0.05, (B, N, 3)), ring=ring, dt=1e-3, horizon=H, stride=3, pins=None if ring else [0],
+                     material=dict(alpha=1e-4, gamma=0.05, stretch=1e-7))
+    P["loss"] = dict(kind="polyline", target=np.zeros((B, 3, N)))
+    got, ref = both_gradients(dlo, orc, P, H, 3)
+    # The compliance entry of g_material is a sum of nearly cancelling terms (w_j gbar_j - w_n gbar_n along each edge); for
+    # ropes of a handful of vertices its true value (1e-2) is of the size of the fp32 cancellation error (1e-3 ... 1e-2, the
+    # same absolute error at N = 24 where the value is 10), so it is compared on the bending and damping entries here.
+    for g in (got, ref):
+        g["g_material"] = g["g_material"][:, 1:3]
+    check("N=%d ring=%s" % (N, ring), got, ref, ("g_x0", "g_v0", "g_material"))

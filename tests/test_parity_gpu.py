@@ -101,3 +101,69 @@ def test_empty_horizon_and_call_order(dlo):
         sim.backward(np.zeros((1, 3, 32)))
     assert e.value.status == -2
     sim.close()
+
+
+# ---- edge cases: smallest and largest ropes, degenerate scenes, error behaviour ---------------------------------------
+def _plain_rope(N, ring, B=3, H=25, seed=3, **cfg):
+    from helpers import rope_problem
+    rng = np.random.default_rng(seed)
+    if ring:
+        th = np.linspace(0, 2 * np.pi, N, endpoint=False)
+        x = np.stack([0.1 * np.cos(th), 0.1 * np.sin(th), 0.02 * np.sin(2 * th)], 1)
+    else:
+        x = np.stack([np.arange(N) * (0.5 / max(N - 1, 1)), np.zeros(N), np.zeros(N)], 1)
+    x = x[None].repeat(B, 0) + rng.normal(0, 2e-4, (B, N, 3))
+    v = rng.normal(0, 0.05, (B, N, 3))
+    pins = None if ring else [0]
+    return rope_problem(x, v, ring=ring, dt=1e-3, horizon=H, pins=pins, material=dict(alpha=1e-4, gamma=0.05, stretch=1e-7), **cfg)
+
+
+@pytest.mark.parametrize("N,ring", [(3, False), (4, True), (5, True), (256, False), (255, True), (64, False), (65, False)],
+                         ids=["N=3 open (minimum)", "N=4 ring (minimum)", "N=5 odd ring", "N=256 open (maximum)", "N=255 odd ring",
+                              "N=64 (full warp at VPL 2)", "N=65 (first size at VPL 4)"])
+def test_extreme_sizes(dlo, orc, N, ring):
+    P = _plain_rope(N, ring, H=15 if N > 200 else 25)
+    got, ref = run_both(dlo, orc, P)
+    err = position_error(P, got["x"], ref["x"])
+    print(summarize("N=%d ring=%s" % (N, ring), err))
+    assert err.max() <= POS_TOL
+
+
+def test_no_projection_iterations_and_no_substep_split(dlo, orc):
+    """N_C = 0 (pure symplectic Euler on the energies) and n_substeps = 1"""
+    P = _plain_rope(20, False, n_proj_iters=0, n_substeps=1, stretch_mode=0)
+    P["material"]["stretch"][:] = 50.0
+    got, ref = run_both(dlo, orc, P)
+    assert position_error(P, got["x"], ref["x"]).max() <= POS_TOL
+
+
+def test_argument_and_order_errors(dlo):
+    import torch
+    P = make_problem(2, batch=4, n_verts=16, horizon=10)
+    sim = dlo.DloSim(P)
+    with pytest.raises(dlo.DloError) as e:          # horizon beyond the actions given
+        dlo.dlo_rollout_forward(sim.h, 11, 0)
+    assert e.value.status == -1
+    with pytest.raises(dlo.DloError) as e:          # negative stride
+        dlo.dlo_rollout_forward(sim.h, 5, -1)
+    assert e.value.status == -1
+    sim.rollout(10, 0)
+    with pytest.raises(dlo.DloError) as e:          # backward without checkpoints
+        sim.backward(np.zeros((4, 3, 16)))
+    assert e.value.status == -2
+    # changing the scene invalidates the state until dlo_set_state is called again
+    dlo.dlo_set_pins(sim.h, torch.zeros((4, 16), dtype=torch.uint8, device="cuda"))
+    with pytest.raises(dlo.DloError) as e:
+        dlo.dlo_rollout_forward(sim.h, 5, 0)
+    assert e.value.status == -2
+    assert sim.n_bad() == 0
+    sim.close()
+
+
+def test_non_finite_state_is_flagged(dlo):
+    P = make_problem(1)
+    P["x0"][0, 0, 5] = np.nan
+    sim = dlo.DloSim(P)
+    sim.rollout(3, 0)
+    assert sim.n_bad() == 1
+    sim.close()
