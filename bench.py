@@ -32,6 +32,10 @@ UNIT = "env-steps/s"
 # in DESIGN.md section 7 (FADD/FMUL = 1, FFMA = 2): forward 0.10 Mflop per substep = 0.5 Mflop per env-step; the reverse of a
 # substep 0.17 Mflop; forward+backward = forward + replay + reverse = 0.5 + 0.5 + 0.85 = 1.85 Mflop per env-step.
 FLOPS_PER_ENV_STEP = {"fwd": 0.5e6, "fwdbwd": 1.85e6}
+# DRAM bytes per env-substep of the dominant kernel (k_adjoint), from the `ncu --set full` capture summarised in
+# profiles/r01_final_ncu_summary.md: (6.623 GB read + 0.305 GB written) / (4096 envs x 20 frames x 5 substeps) = 16.9 KB,
+# against 16.4 KB of tape record it has to read (algorithmic).
+ADJ_DRAM_BYTES_PER_ENV_SUBSTEP = (6.623276e9 + 0.304938e9) / (4096 * 20 * 5)
 # fp32 ALU peak derived in DESIGN.md section 7: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
@@ -255,7 +259,9 @@ def main():
     achieved = flops / (min(per) * 1e-3) / 1e12
     line = dict(base, value=value, ms_per_step=ms_per_step, e2e=e2e, gpu_launches=int(launches), clocks=clocks,
                 roofline={"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS,
-                          "traffic": None, "peak_source": "derived (148 SMs x 128 fp32 lanes x 2 x %.0f MHz, DESIGN.md section 7); HBM peak %s %.0f GB/s" % (
+                          "traffic": (ADJ_DRAM_BYTES_PER_ENV_SUBSTEP * B * max(stride, 1) * 5 if args.mode == "fwdbwd" else None),
+                          "traffic_note": "DRAM bytes per k_adjoint launch (one checkpoint segment), ncu capture in profiles/r01_final_ncu_summary.md",
+                          "peak_source": "derived (148 SMs x 128 fp32 lanes x 2 x %.0f MHz, DESIGN.md section 7); HBM peak %s %.0f GB/s" % (
                               peaks.get("sm_max_mhz", 1965.0), which, peaks.get("hbm_gbs", 0.0)),
                           "kernel": "k_forward" if args.mode == "fwd" else "k_forward + k_adjoint",
                           "algorithmic_flops_per_env_step": FLOPS_PER_ENV_STEP[args.mode]},
