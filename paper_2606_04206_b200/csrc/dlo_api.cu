@@ -36,7 +36,10 @@ struct dlo_sim {
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
   float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
-  uint8_t *kin = nullptr, *pins = nullptr, *tape_flag = nullptr;
+  uint8_t *kin = nullptr, *pins = nullptr, *tape_flag = nullptr, *tape_flag2 = nullptr;
+  float* tape2 = nullptr;            // second tape buffer: the replay of segment g-1 overlaps the adjoint of segment g
+  cudaStream_t aux = nullptr;
+  cudaEvent_t ev_fwd = nullptr, ev_rep[2] = {nullptr, nullptr}, ev_adj[2] = {nullptr, nullptr};
   int *grasp = nullptr, *flags = nullptr;
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
@@ -116,7 +119,8 @@ size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
   n += 2 * B * blk;                                                            // state, state0
   if (stride > 0 && horizon > 0) {
     n += ((size_t)horizon / stride + 1) * B * blk;                             // checkpoints
-    n += ((size_t)(stride < horizon ? stride : horizon) * P.n_sub + 1) * B * tape_rows(P.N_C) * P.NS * sizeof(float);   // tape of one segment
+    const size_t tape = ((size_t)(stride < horizon ? stride : horizon) * P.n_sub + 1) * B * tape_rows(P.N_C) * P.NS * sizeof(float);
+    n += tape * (horizon > stride ? 2 : 1);                                     // tape of one segment, double-buffered when there are several
     n += B * blk;                                                              // running adjoint
     if (P.self_contact) n += B * (size_t)P.N_C * 3 * 33 * vpl_for(P.N) * 4;    // self-contact correction tape
   }
@@ -213,8 +217,10 @@ dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag};
+                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2};
   for (void* p : dev) if (p) cudaFree(p);
+  if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
+  for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
   void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hseed_x, s->hseed_v, s->hg_act, s->hg_x0, s->hg_v0, s->hg_mat, s->hxT, s->hvT};
   for (void* p : host) if (p) cudaFreeHost(p);
   delete s;
@@ -289,18 +295,18 @@ dlo_status dlo_set_actions(dlo_sim* s, const float* actions, int32_t horizon) {
 
 }  // extern "C"
 
-template <int VPL, bool TAPE> static cudaError_t launch_forward_t(dlo_sim* s, const KParams& P, int t0, int t1, int stride) {
+template <int VPL, bool TAPE> static cudaError_t launch_forward_t(dlo_sim* s, const KParams& P, int t0, int t1, int stride, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(k_forward<VPL, TAPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fwd > 48 * 1024 ? s->smem_fwd : 48 * 1024);
   if (e != cudaSuccess) return e;
   const int grid = (P.B + s->wpb_fwd - 1) / s->wpb_fwd;
-  k_forward<VPL, TAPE><<<grid, s->wpb_fwd * 32, s->smem_fwd, s->stream>>>(P, t0, t1, stride);
+  k_forward<VPL, TAPE><<<grid, s->wpb_fwd * 32, s->smem_fwd, st>>>(P, t0, t1, stride);
   s->launches += 1;
   return cudaGetLastError();
 }
 // forward (tape = false) or replay of a segment with tape records (tape = true); P carries the buffers to use
-static cudaError_t launch_forward(dlo_sim* s, KParams P, int t0, int t1, int stride, bool tape) {
+static cudaError_t launch_forward(dlo_sim* s, KParams P, int t0, int t1, int stride, bool tape, cudaStream_t st) {
   smem_layout(P, s->VPL, false);
-#define DLO_FWD_CASE(V) return tape ? launch_forward_t<V, true>(s, P, t0, t1, stride) : launch_forward_t<V, false>(s, P, t0, t1, stride)
+#define DLO_FWD_CASE(V) return tape ? launch_forward_t<V, true>(s, P, t0, t1, stride, st) : launch_forward_t<V, false>(s, P, t0, t1, stride, st)
   switch (s->VPL) {
 #ifdef DLO_VPL_ONLY   /* development builds: one instantiation only */
     default: DLO_FWD_CASE(DLO_VPL_ONLY);
@@ -337,7 +343,7 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     s->P.ckpt = s->ckpt;
     CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
   }
-  if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false));
+  if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false, s->stream));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;
 }

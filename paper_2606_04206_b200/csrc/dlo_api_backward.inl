@@ -51,17 +51,53 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   CU(cudaMemsetAsync(s->gmat, 0, (size_t)B * 5 * sizeof(float), s->stream));
   if (g_actions && s->P.G > 0) CU(cudaMemsetAsync(g_actions, 0, (size_t)H * B * s->P.G * 6 * sizeof(float), s->stream));
   const int nseg = (H + stride - 1) / stride;
-  for (int g = nseg - 1; g >= 0; --g) {
-    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H;
-    CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
-    // replay the segment from its checkpoint, leaving the state at the start of every substep on the tape
+  // Two tape buffers when there is more than one segment and memory allows: the replay of segment g-1 (auxiliary stream)
+  // then overlaps the adjoint of segment g and fills the SMs its last, partly empty wave leaves idle.
+  if (nseg > 1 && !s->tape2) {
+    if (cudaMalloc((void**)&s->tape2, seg * B * rec * sizeof(float)) != cudaSuccess || cudaMalloc((void**)&s->tape_flag2, seg * B) != cudaSuccess) {
+      cudaGetLastError();
+      if (s->tape2) { cudaFree(s->tape2); s->tape2 = nullptr; }
+    }
+  }
+  const bool overlap = nseg > 1 && s->tape2 && s->tape_flag2;
+  if (overlap && !s->aux) {
+    CU(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
+    CU(cudaEventCreateWithFlags(&s->ev_fwd, cudaEventDisableTiming));
+    for (int k = 0; k < 2; ++k) { CU(cudaEventCreateWithFlags(&s->ev_rep[k], cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&s->ev_adj[k], cudaEventDisableTiming)); }
+  }
+  float* tapes[2] = {s->tape, overlap ? s->tape2 : s->tape};
+  uint8_t* tflags[2] = {s->tape_flag, overlap ? s->tape_flag2 : s->tape_flag};
+  cudaStream_t rs = overlap ? s->aux : s->stream;        // stream of the replays
+  auto replay = [&](int g) -> dlo_status {
+    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = overlap ? (g & 1) : 0;
+    CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, rs));
     KParams Pf = s->P;
-    Pf.state = s->replay; Pf.tape = s->tape; Pf.tape_flag = s->tape_flag;
-    CU(launch_forward(s, Pf, t0, t1, 0, true));
+    Pf.state = s->replay; Pf.tape = tapes[buf]; Pf.tape_flag = tflags[buf];
+    CU(launch_forward(s, Pf, t0, t1, 0, true, rs));
+    if (overlap) CU(cudaEventRecord(s->ev_rep[buf], rs));
+    return DLO_OK;
+  };
+  if (overlap) {   // the replays read the checkpoints the forward rollout wrote on the main stream
+    CU(cudaEventRecord(s->ev_fwd, s->stream));
+    CU(cudaStreamWaitEvent(s->aux, s->ev_fwd, 0));
+  }
+  dlo_status rst = replay(nseg - 1);
+  if (rst) return rst;
+  for (int g = nseg - 1; g >= 0; --g) {
+    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = overlap ? (g & 1) : 0;
+    if (overlap) {
+      CU(cudaStreamWaitEvent(s->stream, s->ev_rep[buf], 0));
+      if (g > 0) {   // next replay goes into the other buffer, free once the adjoint of segment g+1 is done with it
+        if (g + 1 <= nseg - 1) CU(cudaStreamWaitEvent(s->aux, s->ev_adj[(g - 1) & 1], 0));
+        if ((rst = replay(g - 1))) return rst;
+      }
+    }
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
-    Pa.tape = s->tape; Pa.tape_flag = s->tape_flag; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
+    Pa.tape = tapes[buf]; Pa.tape_flag = tflags[buf]; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
     CU(launch_adjoint(s, Pa, t0, t1));
+    if (overlap) CU(cudaEventRecord(s->ev_adj[buf], s->stream));
+    else if (g > 0 && (rst = replay(g - 1))) return rst;
   }
   if (g_x0 || g_v0) {
     const size_t n = (size_t)B * STATE_ROWS * s->P.N;

@@ -47,7 +47,7 @@ def test_scratch_bytes_matches_layout(dlo):
     B, N, H, S = 4096, 128, 1000, 100
     blk = 11 * N * 4
     n = dlo.dlo_scratch_bytes(cfg, H, S)
-    ckpt, tape = (H // S + 1) * B * blk, (S * 5 + 1) * B * (22 + 10) * N * 4     # tape record: 22 + N_C rows
+    ckpt, tape = (H // S + 1) * B * blk, 2 * (S * 5 + 1) * B * (22 + 10) * N * 4     # two tape buffers of 22 + N_C rows per record
     assert n > ckpt + tape and n < ckpt + tape + 400e6
     assert dlo.dlo_scratch_bytes(cfg, H, 0) < 100e6          # forward only: constants + two state copies
     bad = make_config(dict(P["config"], n_verts=1000))
