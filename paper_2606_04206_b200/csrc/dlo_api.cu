@@ -44,6 +44,7 @@ struct dlo_sim {
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
   int H_actions = 0, H_done = 0, stride = 0;
+  int tape_seg = -1;               // segment whose tape records are in the buffer already (written by the forward rollout)
   bool have_state = false, have_prims = false, have_grippers = false;
   int64_t launches = 0;
   // staging for the *_host calls
@@ -320,6 +321,30 @@ static cudaError_t launch_forward(dlo_sim* s, KParams P, int t0, int t1, int str
 #undef DLO_FWD_CASE
 }
 
+// tape buffers of one checkpoint segment (two when there are several segments and memory allows: DESIGN.md section 5)
+static dlo_status ensure_tape(dlo_sim* s, int H, int stride) {
+  const int B = s->P.B;
+  const size_t rec = (size_t)tape_rows(s->P.N_C) * s->P.NS, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub + 1;
+  const int nseg = (H + stride - 1) / stride;
+  if (seg > s->tape_blocks) {
+    CU(cudaStreamSynchronize(s->stream));
+    if (s->aux) CU(cudaStreamSynchronize(s->aux));
+    for (void* p : {(void*)s->tape, (void*)s->tape2, (void*)s->tape_flag, (void*)s->tape_flag2}) if (p) cudaFree(p);
+    s->tape = s->tape2 = nullptr; s->tape_flag = s->tape_flag2 = nullptr; s->tape_blocks = 0;
+    CU(dalloc(&s->tape, seg * B * rec));
+    CU(dalloc(&s->tape_flag, seg * B));
+    s->tape_blocks = seg;
+  }
+  if (nseg > 1 && !s->tape2) {
+    if (cudaMalloc((void**)&s->tape2, s->tape_blocks * B * rec * sizeof(float)) != cudaSuccess ||
+        cudaMalloc((void**)&s->tape_flag2, s->tape_blocks * B) != cudaSuccess) {
+      cudaGetLastError();
+      if (s->tape2) { cudaFree(s->tape2); s->tape2 = nullptr; }
+    }
+  }
+  return DLO_OK;
+}
+
 extern "C" {
 
 dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
@@ -343,7 +368,20 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     s->P.ckpt = s->ckpt;
     CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
   }
-  if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false, s->stream));
+  s->tape_seg = -1;
+  if (horizon > 0 && stride > 0) {
+    // the last segment is run in tape mode, so that the reverse pass can start without replaying it
+    dlo_status st = ensure_tape(s, horizon, stride);
+    if (st) return st;
+    const int nseg = (horizon + stride - 1) / stride, t_last = (nseg - 1) * stride;
+    const bool two = nseg > 1 && s->tape2 && s->tape_flag2;
+    if (t_last > 0) CU(launch_forward(s, s->P, 0, t_last, stride, false, s->stream));
+    KParams Pf = s->P;
+    Pf.tape = (two && ((nseg - 1) & 1)) ? s->tape2 : s->tape;
+    Pf.tape_flag = (two && ((nseg - 1) & 1)) ? s->tape_flag2 : s->tape_flag;
+    CU(launch_forward(s, Pf, t_last, horizon, stride, true, s->stream));
+    s->tape_seg = nseg - 1;
+  } else if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false, s->stream));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;
 }

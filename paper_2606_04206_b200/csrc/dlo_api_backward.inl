@@ -28,15 +28,9 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
   const int H = s->H_done, stride = s->stride, B = s->P.B;
   const size_t blk = s->blk, rec = (size_t)tape_rows(s->P.N_C) * s->P.NS, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub + 1;
-  if (seg > s->tape_blocks) {
-    CU(cudaStreamSynchronize(s->stream));
-    if (s->tape) cudaFree(s->tape);
-    s->tape = nullptr; s->tape_blocks = 0;
-    CU(dalloc(&s->tape, seg * B * rec));
-    if (s->tape_flag) cudaFree(s->tape_flag);
-    s->tape_flag = nullptr;
-    CU(dalloc(&s->tape_flag, seg * B));
-    s->tape_blocks = seg;
+  {
+    dlo_status st = ensure_tape(s, H, stride);
+    if (st) return st;
   }
   if (!s->adj) {
     CU(dalloc(&s->adj, (size_t)B * blk));
@@ -53,12 +47,6 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   const int nseg = (H + stride - 1) / stride;
   // Two tape buffers when there is more than one segment and memory allows: the replay of segment g-1 (auxiliary stream)
   // then overlaps the adjoint of segment g and fills the SMs its last, partly empty wave leaves idle.
-  if (nseg > 1 && !s->tape2) {
-    if (cudaMalloc((void**)&s->tape2, seg * B * rec * sizeof(float)) != cudaSuccess || cudaMalloc((void**)&s->tape_flag2, seg * B) != cudaSuccess) {
-      cudaGetLastError();
-      if (s->tape2) { cudaFree(s->tape2); s->tape2 = nullptr; }
-    }
-  }
   const bool overlap = nseg > 1 && s->tape2 && s->tape_flag2;
   if (overlap && !s->aux) {
     CU(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
@@ -81,12 +69,14 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaEventRecord(s->ev_fwd, s->stream));
     CU(cudaStreamWaitEvent(s->aux, s->ev_fwd, 0));
   }
-  dlo_status rst = replay(nseg - 1);
-  if (rst) return rst;
+  dlo_status rst = DLO_OK;
+  if (s->tape_seg != nseg - 1 && (rst = replay(nseg - 1))) return rst;     // normally the forward rollout left it on the tape
+  const bool have_last = s->tape_seg == nseg - 1;
+  s->tape_seg = -1;
   for (int g = nseg - 1; g >= 0; --g) {
     const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = overlap ? (g & 1) : 0;
     if (overlap) {
-      CU(cudaStreamWaitEvent(s->stream, s->ev_rep[buf], 0));
+      if (!(have_last && g == nseg - 1)) CU(cudaStreamWaitEvent(s->stream, s->ev_rep[buf], 0));
       if (g > 0) {   // next replay goes into the other buffer, free once the adjoint of segment g+1 is done with it
         if (g + 1 <= nseg - 1) CU(cudaStreamWaitEvent(s->aux, s->ev_adj[(g - 1) & 1], 0));
         if ((rst = replay(g - 1))) return rst;
