@@ -50,15 +50,25 @@ template <int VPL> struct SubRec {
 };
 
 // A1 (L129, R-20): lane g < G evaluates gripper g at the substep's start and end and publishes it
-__device__ __forceinline__ void publish_poses(const KParams& P, int env, int lane, const float ap[6], const float ac[6], int s, float* pose_sm) {
+// `chain`: the block still holds the previous substep of the same step, whose end pose is this substep's start pose
+__device__ __forceinline__ void publish_poses(const KParams& P, int env, int lane, const float ap[6], const float ac[6], int s, float* pose_sm,
+                                              bool chain = false) {
   if (lane < P.G) {
     const float tau0 = (float)s / (float)P.n_sub, tau1 = (float)(s + 1) / (float)P.n_sub;
-    Pose<float> g0 = make_pose<float>(ap, ac, tau0), g1 = make_pose<float>(ap, ac, tau1);
     float* o = pose_sm + lane * POSE_STRIDE;
-    o[POSE_P0] = g0.p.x; o[POSE_P0 + 1] = g0.p.y; o[POSE_P0 + 2] = g0.p.z;
+    if (chain) {
+#pragma unroll
+      for (int k = 0; k < 12; ++k) o[POSE_P0 + k] = o[POSE_P1 + k];   // p1, R1 -> p0, R0 (contiguous)
+    } else {
+      const Pose<float> g0 = make_pose<float>(ap, ac, tau0);
+      o[POSE_P0] = g0.p.x; o[POSE_P0 + 1] = g0.p.y; o[POSE_P0 + 2] = g0.p.z;
+#pragma unroll
+      for (int k = 0; k < 9; ++k) o[POSE_R0 + k] = g0.R.m[k];
+    }
+    const Pose<float> g1 = make_pose<float>(ap, ac, tau1);
     o[POSE_P1] = g1.p.x; o[POSE_P1 + 1] = g1.p.y; o[POSE_P1 + 2] = g1.p.z;
 #pragma unroll
-    for (int k = 0; k < 9; ++k) { o[POSE_R0 + k] = g0.R.m[k]; o[POSE_R1 + k] = g1.R.m[k]; }
+    for (int k = 0; k < 9; ++k) o[POSE_R1 + k] = g1.R.m[k];
     const float* fg = P.finger + ((size_t)env * P.G + lane) * 4;
     const float gap = fg[0], len = fg[1];
     f3 A0 = g1.p + mul(g1.R, mk3<float>(0.5f * gap, 0.f, 0.f)), B0 = g1.p + mul(g1.R, mk3<float>(0.5f * gap, 0.f, len));
@@ -374,7 +384,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   constexpr bool REC = MODE == 1;
   const float h = P.h, inv_h = P.inv_h;
   // -- A1 bodies
-  if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);
+  if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose, MODE != 1 && sub > 0);
 
   phase_sync(sm);
   // -- A2 forces: gravity, stretch (mode ENERGY, Eq.2-3), bending (Eq.4-7)
