@@ -182,3 +182,48 @@ def test_gradient_extreme_sizes(dlo, orc, N, ring):
     for g in (got, ref):
         g["g_material"] = g["g_material"][:, 1:3]
     check("N=%d ring=%s" % (N, ring), got, ref, ("g_x0", "g_v0", "g_material"))
+
+
+def test_rope_landing_on_box_and_cylinder(dlo, orc):
+    """a short rope falls onto a rotated box, a lying cylinder and a thin capsule between them: exercises the box, cylinder
+    and capsule SDF branches and their adjoints in contact, with friction"""
+    from helpers import rope_problem
+    from parity import POS_TOL, position_error
+    rng = np.random.default_rng(21)
+    B, N, H = 4, 20, 32
+    x = np.stack([np.linspace(-0.08, 0.08, N), np.zeros(N), np.full(N, 0.058)], 1)
+    x = x[None].repeat(B, 0) + rng.normal(0, 3e-4, (B, N, 3))
+    x[:, :, 1] += rng.uniform(-0.01, 0.01, (B, 1))
+    v = np.zeros_like(x)
+    v[..., 2] = -0.3
+    v[..., 0] = 0.2
+    P = rope_problem(x, v, dt=1e-3, horizon=H, stride=9, n_primitives=3, material=dict(alpha=3e-4, gamma=0.05, stretch=1e-7, mu_r=0.4))
+    P["prim_types"] = np.array([3, 2, 1], dtype=np.int32)
+    pp = np.zeros((B, 3, 10))
+    pp[:, 0, 0:3] = (-0.04, 0.0, 0.025)                    # box: centre, half extents, rotation vector (tilted and yawed)
+    pp[:, 0, 3:6] = (0.03, 0.03, 0.025)
+    pp[:, 0, 6:9] = (0.1, -0.15, 0.4)
+    pp[:, 1, 0:3] = (0.05, 0.0, 0.03)                      # cylinder lying along y: centre, axis, radius, half height
+    pp[:, 1, 3:6] = (0.0, 1.0, 0.0)
+    pp[:, 1, 6], pp[:, 1, 7] = 0.022, 0.05
+    pp[:, 2, 0:3] = (0.0, -0.03, 0.046)                     # capsule across the gap between them: end points, radius
+    pp[:, 2, 3:6] = (0.01, 0.03, 0.05)
+    pp[:, 2, 6] = 0.004
+    P["prim_params"] = pp
+    P["loss"] = dict(kind="polyline", target=np.zeros((B, 3, N)))
+    free = dict(P, config=dict(P["config"], n_primitives=0))
+    a, b = orc.OracleSim(P).rollout(H, 0)["x"], orc.OracleSim(free).rollout(H, 0)["x"]
+    assert np.abs(a - b).max() > 2e-3, "the rope must actually land on the bodies"
+    sim = dlo.DloSim(P)
+    xg = sim.rollout(H, 0).state()["x"]
+    sim.close()
+    err = position_error(P, xg, a)
+    print(summarize("box+cylinder positions", err))
+    assert err.max() <= POS_TOL
+    got, ref = both_gradients(dlo, orc, P, H, 9)
+    for k in ("g_x0", "g_v0", "g_material"):
+        e = gradient_error(got[k], ref[k])
+        print(summarize("box+cylinder+capsule " + k, e))
+        # contact with thin bodies puts an env on a branch threshold now and then (see KINKED above): three of the four envs
+        # must meet the plain bar, the fourth stay within 1e-2
+        assert np.sort(e)[-2] <= GRAD_TOL and e.max() <= 1e-2, (k, e)
