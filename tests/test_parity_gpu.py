@@ -167,3 +167,69 @@ def test_non_finite_state_is_flagged(dlo):
     sim.rollout(3, 0)
     assert sim.n_bad() == 1
     sim.close()
+
+
+def test_host_buffer_calls_match_device_calls(dlo):
+    """dlo_rollout_forward_host / dlo_backward_host (the e2e path of bench.py) give the same bits as the device-pointer calls"""
+    P = make_problem(3, batch=8, n_verts=24, horizon=20, stride=7)
+    from parity import loss_and_seed
+    sim = dlo.DloSim(P)
+    xd = sim.rollout(20, 7).state()["x"]
+    _, seed = loss_and_seed(P, xd)
+    gd = sim.backward(seed)
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    x0, v0, act = f32(P["x0"]), f32(P["v0"]), f32(P["actions"])
+    xT, vT = np.empty_like(x0), np.empty_like(x0)
+    dlo.dlo_rollout_forward_host(sim.h, x0, v0, None, act, 20, 7, xT, vT)
+    assert np.array_equal(xT.astype(np.float64), xd)
+    ga, gx, gv, gm = np.empty_like(act), np.empty_like(x0), np.empty_like(x0), np.empty((8, 5), dtype=np.float32)
+    dlo.dlo_backward_host(sim.h, f32(seed), None, ga, gx, gv, gm)
+    assert np.allclose(gx, gd["g_x0"], rtol=1e-5, atol=1e-9) and np.allclose(gv, gd["g_v0"], rtol=1e-5, atol=1e-9)
+    assert np.allclose(ga, gd["g_actions"], rtol=1e-4, atol=1e-7 * np.abs(gd["g_actions"]).max())
+    sim.close()
+
+
+def test_trajectory_matches_oracle_at_every_recorded_time(dlo, orc):
+    """not only the final state: the state after 1, 2, 7, 23 and 60 frames (ring on posts with a gripper, config 4)"""
+    P = make_problem(4, batch=4, n_verts=48, horizon=60)
+    o = orc.OracleSim(P)
+    o.rollout(60, 0, record=True)
+    sim = dlo.DloSim(P)
+    for t in (1, 2, 7, 23, 60):
+        got = sim.rollout(t, 0).state()
+        ref = o.record(t)
+        assert position_error(P, got["x"], ref["x"]).max() <= POS_TOL, t
+        assert np.abs(got["v"] - ref["v"]).max() <= 1e-3 * max(1.0, np.abs(ref["v"]).max()), t
+    sim.close()
+    o.close()
+
+
+def test_rest_shape_is_stationary_on_the_gpu(dlo, orc):
+    """a curved rope / a non-planar ring whose rest curvature is its own shape (kappa_bar_from_x0), no gravity: nothing moves
+    (pin C-7 of the oracle, here for the CUDA path: frames, Eq.12 and the bending force are consistent)"""
+    from helpers import rope_problem
+    for ring in (False, True):
+        N = 40
+        if ring:
+            th = np.linspace(0, 2 * np.pi, N, endpoint=False)
+            x = np.stack([0.1 * np.cos(th), 0.1 * np.sin(th), 0.02 * np.sin(2 * th)], 1)
+        else:
+            s = np.linspace(0, 1, N)
+            x = np.stack([0.3 * s, 0.05 * np.sin(3 * s), 0.04 * np.cos(2 * s)], 1)
+        if not ring:      # equal edge lengths so that the stretch constraints are satisfied too
+            from workloads.configs import _resample_polyline
+            x = _resample_polyline(x, N)
+        P = rope_problem(x[None], ring=ring, dt=1e-3, horizon=50, gravity=(0.0, 0.0, 0.0), kappa_bar_from_x0=1,
+                         material=dict(alpha=1e-3, stretch=1e-5))
+        sim = dlo.DloSim(P)
+        got = sim.rollout(50, 0).state()
+        sim.close()
+        ref = orc.OracleSim(P).rollout(50, 0)
+        L = np.linalg.norm(np.diff(x, axis=0), axis=1).sum()
+        moved_gpu = np.linalg.norm(got["x"][0].T - x, axis=1).max()
+        moved_orc = np.linalg.norm(ref["x"][0].T - x, axis=1).max()
+        # the oracle itself moves only by the residual of unequal chord lengths against the mean rest length
+        assert moved_gpu <= moved_orc + 2e-5 * L, (ring, moved_gpu, moved_orc)
+        assert position_error(P, got["x"], ref["x"]).max() <= POS_TOL
+        if not ring:
+            assert moved_gpu <= 2e-5 * L
