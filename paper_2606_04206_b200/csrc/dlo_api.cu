@@ -65,15 +65,19 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
   P.sm_prim = take(P.K * PRIM_SM_STRIDE);
   P.sm_q = take(P.G * P.M * 3);
   P.sm_ys = P.sm_acc = P.sm_vs = P.sm_mid = P.sm_dp = P.sm_cand = 0;
-  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = P.sm_blk = 0;
+  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = P.sm_blk = P.sm_xref = 0;
   if (P.self_contact) {
     P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
     P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap);   // candidates + prefilter survivors (ushort each)
     P.sm_blk = take(4 * 32);
+    if (!adjoint) P.sm_xref = take(3 * NP);   // positions at which the pair list was built (must outlive the substep)
   }
   if (adjoint) {
     P.sm_posebar = take(P.G * 24);
-    if (P.self_contact) { P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP); }
+    if (P.self_contact) {
+      P.sm_dpbar = take(P.cand_cap); P.sm_ybar = take(3 * NP); P.sm_vbar = take(3 * NP);
+      P.sm_xref = P.sm_ybar;   // the reverse pass rebuilds the pair list in every recomputed substep; ybar is zeroed before each use
+    }
   }
   P.sm_warp_floats = o;
   return o * (int)sizeof(float);   // bytes per warp
@@ -105,6 +109,7 @@ static void fill_params(const dlo_config& c, KParams& P) {
   P.self_contact = c.enable_self_contact != 0; P.self_skip = c.self_skip;
   P.G = c.n_grippers; P.M = P.G ? c.n_grasp_max : 1; P.K = c.n_primitives;
   P.cand_cap = round_up(4 * P.N, 32);
+  P.list_margin = c.rope_radius;   // a quarter of the candidate distance 2(r_a+r_b)
   P.h = c.dt / (float)c.n_substeps; P.inv_h = 1.0f / P.h;
   for (int k = 0; k < 3; ++k) P.g[k] = c.gravity[k];
   P.r = c.rope_radius; P.inv_eps = 1.0f / c.contact_softness; P.f_thresh = c.influence_threshold; P.e_rest = c.restitution;

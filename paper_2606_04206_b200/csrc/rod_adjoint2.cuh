@@ -68,8 +68,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
     edge_refresh<VPL>(tp, s, ec);
     edge_prev_refresh<VPL>(tp, s, ec);
-#pragma unroll
-    for (int q = 0; q < SUBSTEP_SYNCS; ++q) phase_sync(sm);
+    substep_idle_syncs(sm);
   }
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
 

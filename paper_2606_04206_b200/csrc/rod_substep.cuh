@@ -7,7 +7,7 @@
 namespace dlo {
 
 struct WarpSmem {
-  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk;
+  float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk, *xref;
   unsigned short* cand;
   float* base;        // the warp's shared-memory block (non-inlined helpers rebuild the view from this one pointer)
   int sync_threads;   // > 0: warps of the CTA walk the phases in lockstep (named barrier over this many threads)
@@ -15,7 +15,7 @@ struct WarpSmem {
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
-    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk;
+    lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk; xref = base + P.sm_xref;
     NP = np;
     this->base = base;
     sync_threads = 0;
@@ -28,15 +28,27 @@ __device__ __forceinline__ void phase_sync(const WarpSmem& sm) {
   if (sm.sync_threads > 0) asm volatile("bar.sync 1, %0;" ::"r"(sm.sync_threads) : "memory");
 }
 
+// Phase barrier that also ORs a per-thread flag over the CTA (bar.red): the warps decide together, at no extra cost
+__device__ __forceinline__ bool phase_vote(const WarpSmem& sm, bool v) {
+  if (sm.sync_threads <= 0) return v;
+  int r;
+  asm volatile(
+      "{\n\t.reg .pred pin, pout;\n\tsetp.ne.s32 pin, %2, 0;\n\tbar.red.or.pred pout, 1, %1, pin;\n\tselp.s32 %0, 1, 0, pout;\n\t}"
+      : "=r"(r) : "r"(sm.sync_threads), "r"((int)v) : "memory");
+  return r != 0;
+}
+
 // what is known about self-contact from earlier substeps: positions at which the candidate list was last built and
 // the exact minimum pair distance there (dref < 0: nothing known, build at first need; huge: never build)
 template <int VPL> struct ContactCache {
   f3 xref[VPL];
   float dref;
+  int nlist;   // size of the pair list in shared memory (build_pair_list); < 0: none yet or truncated, rebuild at next use
   __device__ __forceinline__ void reset(float d) {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) xref[k] = zero3<float>();
     dref = d;
+    nlist = -1;
   }
 };
 
@@ -134,19 +146,23 @@ __device__ __forceinline__ float pair_dist2(const float* ys, int NP, int pa, int
 }
 
 // A4 candidate list (Eq.13 "potentially colliding", R-15): all edge pairs a<b with cyclic index distance >=
-// self_skip whose segments are closer than 2(r_a+r_b) at x^p.  The SET equals the oracle's; it is found
-// hierarchically instead of by the all-pairs loop: (1) bounding spheres of the lanes' edge blocks (VPL edges each)
-// are tested pairwise, (2) edge pairs of the surviving block pairs pass a midpoint-sphere prefilter, (3) the
-// survivors take the exact segment-segment test, 32 at a time.  Every rejection is conservative, so no pair is
-// lost.  Order: by (block a, block b, slot a, slot b) - deterministic, but not the oracle's lexicographic order
-// (only the fp32 summation order of the Jacobi pass depends on it).  ys = x^p, mid = (midpoint, half length, w).
-struct CandOut { int ncand; float dmin; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b)
+// self_skip whose segments are closer than 2(r_a+r_b) at x^p.  The SET equals the oracle's; it is found in two
+// stages.  build_pair_list (run only when some vertex has moved more than list_margin since its last run) collects a
+// conservative superset, the pairs that can come within 2(r_a+r_b) while no vertex moves further than list_margin:
+// (1) bounding spheres of the lanes' edge blocks (VPL edges each) are tested pairwise, (2) edge pairs of the
+// surviving block pairs pass a midpoint-sphere test, both with the reach widened by 2 list_margin (segment distance
+// is 1-Lipschitz in the end points).  filter_candidates (every substep that needs the list) takes the exact
+// segment-segment test at x^p over that superset, 32 pairs at a time.  Every rejection is conservative, so no pair
+// is lost.  Order: by (block a, block b, slot a, slot b) - a function of the pair indices only, so the list is the
+// same whenever and wherever the superset was built (forward, replay and the recomputing reverse pass agree bit
+// for bit); it is not the oracle's lexicographic order (only the fp32 summation order of the Jacobi pass depends
+// on it).  mid = (midpoint, half length, w) at the positions the superset was built at.
 template <int VPL>
-__device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, float* smbase, int env, float bx, float by, float bz, float br) {
+__device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* smbase, float slack, float bx, float by, float bz, float br) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
-  const int E = P.E, N = P.N, NP = sm.NP, nb = (E + VPL - 1) / VPL;
-  const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
+  const int E = P.E, NP = sm.NP, nb = (E + VPL - 1) / VPL;
+  const float lim = 4.0f * P.r + slack;   // 2 (r_a + r_b) + slack
   constexpr int PP = VPL * VPL, NPER = PP <= 32 ? 32 / PP : 1, ITER = (PP + 31) / 32;
   unsigned short* surv = sm.cand + P.cand_cap;
   // (1) block pairs: lane B tests its own block against block A
@@ -159,7 +175,7 @@ __device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, flo
     const unsigned m = __ballot_sync(DLO_FULL, hit);
     if (lane == A) mymask = m;
   }
-  // (2) edge pairs of surviving block pairs -> survivors of the midpoint-sphere prefilter
+  // (2) edge pairs of surviving block pairs -> survivors of the midpoint-sphere test
   int nsurv = 0;
   for (int A = 0; A < nb; ++A) {
     unsigned mask = __shfl_sync(DLO_FULL, mymask, A);
@@ -189,10 +205,19 @@ __device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, flo
       for (int q = 0; q < NPER; ++q) mask &= mask - 1u;
     }
   }
-  bool overflow = nsurv > P.cand_cap;
-  nsurv = min(nsurv, P.cand_cap);
   __syncwarp();
-  // (3) exact narrow phase on the survivors, ordered compaction into the candidate list
+  return nsurv;   // > cand_cap: truncated
+}
+
+// exact narrow phase at x^p (in sm.ys) over the pair list, ordered compaction into the candidate list
+struct CandOut { int ncand; float dmin; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b)
+template <int VPL>
+__device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, float* smbase, int nsurv, bool overflow) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
+  const int N = P.N, NP = sm.NP;
+  const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
+  const unsigned short* surv = sm.cand + P.cand_cap;
   int ncand = 0;
   float d2min = lim * lim;
   for (int p0 = 0; p0 < nsurv; p0 += 32) {
@@ -210,7 +235,6 @@ __device__ __noinline__ CandOut build_candidates(const KParams& P, int lane, flo
     if (hit) sm.cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)c;
     ncand += __popc(m);
   }
-  if (overflow && lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
   __syncwarp();
   CandOut out;
   out.ncand = ncand;
@@ -373,8 +397,13 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
 // ---------------------------------------------------------------------------------------------------------
 // One substep.  On entry `ec` holds the edge geometry of s.x (tangents, inverse lengths, previous lane's last
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
-// number of phase_sync() calls inside substep(): a warp that skips the recompute must still take part in them
-enum { SUBSTEP_SYNCS = 4 };
+// the barriers of substep() for a warp that skips the recompute (it must still take part in them, votes included)
+__device__ __forceinline__ void substep_idle_syncs(const WarpSmem& sm) {
+  phase_sync(sm);
+  if (phase_vote(sm, false)) phase_vote(sm, false);
+  phase_sync(sm);
+  phase_sync(sm);
+}
 // MODE 0: plain forward.  MODE 1 (REC): recompute inside the adjoint kernel (contact corrections -> acc_tape).
 // MODE 2 (TAPE): replay of a segment.  In both, the Eq.10 multipliers go to the tape rows `lam_rows` [N_C][NS].
 template <int VPL, int MODE>
@@ -437,32 +466,66 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       if (tp.vvalid[k]) { const f3 d = R.xp[k] - cc.xref[k]; m2 = fmaxf(m2, dot(d, d)); }
     D1 = sqrt_(warp_max(m2));
   }
-  auto build_list = [&]() {
+  auto build_list = [&](bool vote) {
+    // is the pair list still a superset?  (no vertex further than list_margin from where it was built)
+    bool fresh = cc.nlist < 0, overflow = false;
+    int nuse = cc.nlist;
+    if (!fresh) {
+      float m2 = 0.0f;
+#pragma unroll
+      for (int k = 0; k < VPL; ++k)
+        if (tp.vvalid[k]) { const f3 d = R.xp[k] - lds3(sm.xref, sm.NP, vpos<VPL>(tp.base + k)); m2 = fmaxf(m2, dot(d, d)); }
+      const float lm = 0.999f * P.list_margin;
+      const float wm = warp_max(m2);
+      fresh = !(wm <= lm * lm);
+    }
+    if (vote) fresh = phase_vote(sm, fresh) || fresh;   // a warp of the CTA rebuilds: all do (they would wait for it anyway)
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
       const int i = vpos<VPL>(tp.base + k);
       sts3(sm.ys, sm.NP, i, R.xp[k]);
-      sts3(sm.mid, sm.NP, i, axpy(R.xp[k], 0.5f, epred[k]));
-      sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
       sm.mid[4 * sm.NP + i] = c.w[k];
     }
-    // bounding sphere of this lane's edge block (centre = mean of its edge midpoints)
-    f3 bc = zero3<float>();
-    float bn = 0.0f, brad = -1.0e30f;
+    if (fresh) {
 #pragma unroll
-    for (int k = 0; k < VPL; ++k)
-      if (tp.evalid[k]) { bc += axpy(R.xp[k], 0.5f, epred[k]); bn += 1.0f; }
-    if (bn > 0.0f) {
-      bc = (1.0f / bn) * bc;
+      for (int k = 0; k < VPL; ++k) {
+        const int i = vpos<VPL>(tp.base + k);
+        sts3(sm.xref, sm.NP, i, R.xp[k]);
+        sts3(sm.mid, sm.NP, i, axpy(R.xp[k], 0.5f, epred[k]));
+        sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
+      }
+      // bounding sphere of this lane's edge block (centre = mean of its edge midpoints)
+      f3 bc = zero3<float>();
+      float bn = 0.0f, brad = -1.0e30f;
 #pragma unroll
       for (int k = 0; k < VPL; ++k)
-        if (tp.evalid[k]) {
-          const f3 dm = axpy(R.xp[k], 0.5f, epred[k]) - bc;
-          brad = fmaxf(brad, sqrt_(dot(dm, dm)) + 0.5f * sqrt_(dot(epred[k], epred[k])));
+        if (tp.evalid[k]) { bc += axpy(R.xp[k], 0.5f, epred[k]); bn += 1.0f; }
+      if (bn > 0.0f) {
+        bc = (1.0f / bn) * bc;
+#pragma unroll
+        for (int k = 0; k < VPL; ++k)
+          if (tp.evalid[k]) {
+            const f3 dm = axpy(R.xp[k], 0.5f, epred[k]) - bc;
+            brad = fmaxf(brad, sqrt_(dot(dm, dm)) + 0.5f * sqrt_(dot(epred[k], epred[k])));
+          }
+      }
+      __syncwarp();
+      cc.nlist = build_pair_list<VPL>(P, tp.lane, sm.base, 2.0f * P.list_margin, bc.x, bc.y, bc.z, brad);
+      if (cc.nlist > P.cand_cap) {
+        // the superset does not fit (a tightly folded rope): list of this substep's positions only, rebuilt at the next use
+        nuse = build_pair_list<VPL>(P, tp.lane, sm.base, 0.0f, bc.x, bc.y, bc.z, brad);
+        cc.nlist = -1;
+        if (nuse > P.cand_cap) {
+          overflow = true;
+          nuse = P.cand_cap;
+          if (tp.lane == 0) atomicOr(P.flags + env, FLAG_CAND_OVERFLOW);
         }
+      } else {
+        nuse = cc.nlist;
+      }
     }
     __syncwarp();
-    const CandOut co = build_candidates<VPL>(P, tp.lane, sm.base, env, bc.x, bc.y, bc.z, brad);
+    const CandOut co = filter_candidates<VPL>(P, tp.lane, sm.base, nuse, overflow);
     R.ncand = co.ncand;
     cc.dref = co.dmin;
 #pragma unroll
@@ -471,7 +534,17 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     __syncwarp();
   };
 
-  phase_sync(sm);
+  // The warps of a CTA walk in lockstep, so a warp that refreshes its contact data stalls the others: they refresh
+  // together, whenever one of them has to (refreshing early changes no result), which aligns their next refreshes too.
+  {
+    const float need = 2.0f * P.r + 1.0e-6f;
+    const bool want = P.self_contact && !(cc.dref - 2.0f * D1 >= need);
+    if (phase_vote(sm, want) && P.self_contact) {
+      build_list(true);
+      built = true;
+      D1 = 0.0f;
+    }
+  }
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
   for (int it = 0; it < P.N_C; ++it) {
@@ -546,7 +619,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       const float Dm = sqrt_(warp_max(m2)), need = 2.0f * P.r + 1.0e-6f;
       sweep = !(cc.dref - 2.0f * (D1 + Dm) >= need);
       if (sweep && !built) {
-        build_list();
+        build_list(false);
         built = true;
         D1 = 0.0f;
         sweep = !(cc.dref - 2.0f * Dm >= need);
