@@ -169,13 +169,14 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     // (4096 envs on 148 SMs: 7 warps -> 1.98 waves, where 8 warps would leave the second wave 27 % empty)
     int n_sm = 148;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
-    // CTA shape: c warps per CTA, as many CTAs per SM as 16 warps (128 registers) and shared memory allow.  Cost model
+    // CTA shape: c warps per CTA, as many CTAs per SM as the register file (16 warps at 128 registers) and shared memory allow.  Cost model
     // fitted to a sweep on config 5: time ~ waves * sqrt(warps per SM), larger CTAs slightly
     // better at equal occupancy (more warps share each instruction-cache fill).
+    const int max_w = s->VPL <= 4 ? 16 : 8;   // resident warps per SM the register file allows (128 / 255 registers)
     double best = 1e30;
     s->wpb_fwd = 1;
     for (int cw = 1; cw <= DLO_FWD_WARPS; ++cw) {
-      const int k = std::min(16 / cw, cap / std::max(cw * per_fwd, 1));
+      const int k = std::min(max_w / cw, cap / std::max(cw * per_fwd, 1));
       if (k < 1) continue;
       const double slots = (double)k * n_sm * cw, waves = ceil(P.B / slots), cost = waves * sqrt((double)(k * cw)) * (1.0 - 0.01 * cw);
       if (cost < best - 1e-9) { best = cost; s->wpb_fwd = cw; }

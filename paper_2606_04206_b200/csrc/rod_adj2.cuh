@@ -213,9 +213,11 @@ template <class T> DLO_HD void sdf_pre_adj(int type, const T* P, const V3<T>& y,
       for (int k = 0; k < 3; ++k) if (q[k] > T(0)) pb[k] = sg[k] * (phibar * o[k] / phi + (ub[k] - udot * o[k] / phi) / phi);
     } else {
       int k = 0;
-      if (q[1] > q[k]) k = 1;
-      if (q[2] > q[k]) k = 2;
-      pb[k] = sg[k] * phibar;
+      T qk = q[0];
+      if (q[1] > qk) { k = 1; qk = q[1]; }
+      if (q[2] > qk) { k = 2; qk = q[2]; }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) if (j == k) pb[j] = sg[j] * phibar;
     }
     ybar += mul(R, mk3<T>(pb[0], pb[1], pb[2]));
   }

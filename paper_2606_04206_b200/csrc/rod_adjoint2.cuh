@@ -224,8 +224,13 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         const f3 dxr0 = dxr, gr0 = gr;
 #pragma unroll
         for (int k = 0; k < VPL; k += 2) {
-          if (k == tp.ks && tp.base + k == P.E - 1 && c.w[k] + c.wr > 0.0f)
-            edge_reverse(epred[k], lamv[k], c.w[k], c.wr, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
+          // on copies, written back unconditionally: a body guarded by `k == tp.ks` that updates the arrays in place makes
+          // the compiler index them by ks, which puts them in local memory for the whole kernel
+          const bool on = (k == tp.ks) && (tp.base + k == P.E - 1) && (c.w[k] + c.wr > 0.0f);
+          f3 dxk = R.dx[k], dxn = dxr, gk = dxb[k], gn = gr, eb = epb[k];
+          float Sk = R.S[k], sb = Sb[k], ab = atilbar;
+          if (on) edge_reverse(epred[k], lamv[k], c.w[k], c.wr, atil, dxk, dxn, Sk, gk, gn, sb, ab, eb);
+          R.dx[k] = dxk; dxr = dxn; R.S[k] = Sk; dxb[k] = gk; gr = gn; Sb[k] = sb; atilbar = ab; epb[k] = eb;
         }
         R.dx[0] += shfl3(dxr - dxr0, tp.pl);
         dxb[0] += shfl3(gr - gr0, tp.pl);

@@ -187,9 +187,10 @@ template <class T> DLO_HD bool sdf_box(const T* P, const M3<T>& R, const V3<T>& 
     nl = mk3<T>(sg[0] * o0 / phi, sg[1] * o1 / phi, sg[2] * o2 / phi);
   } else {
     int k = 0;
-    if (q[1] > q[k]) k = 1;
-    if (q[2] > q[k]) k = 2;
-    phi = q[k];
+    T qk = q[0];   // (no q[k]: a dynamically indexed array lives in local memory)
+    if (q[1] > qk) { k = 1; qk = q[1]; }
+    if (q[2] > qk) { k = 2; qk = q[2]; }
+    phi = qk;
     nl = mk3<T>(k == 0 ? sg[0] : T(0), k == 1 ? sg[1] : T(0), k == 2 ? sg[2] : T(0));
   }
   n = mul(R, nl);

@@ -588,26 +588,24 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         R.dx[0] -= shfl3(back, tp.pl);
       }
       // third colour: the closing edge of an odd ring (slot ks of the last lane, even slot)
+      // (written like the red sweep, every even slot with a per-slot flag: a body guarded by `k == tp.ks` makes the
+      // compiler index dx / S / epred by ks, which puts those arrays in local memory for the whole kernel)
       if (P.odd_ring) {
         const f3 dxr = shfl3(R.dx[0], tp.nl);
         f3 back = zero3<float>();
-        float lam3 = 0.0f;
 #pragma unroll
         for (int k = 0; k < VPL; k += 2) {
-          if (k == tp.ks && tp.base + k == P.E - 1) {
-            const float wsum = c.w[k] + c.wr;
-            float lam = 0.0f;
-            f3 t = zero3<float>();
-            if (wsum > 0.0f) project_edge<float>(epred[k] + (dxr - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
-            R.S[k] += lam;
-            R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
-            back = (lam * c.wr) * t;
-            lam3 = lam;
-            lamv[k] = lam;   // the closing edge's slot is idle in the red sweep
-          }
+          const bool on = (k == tp.ks) && (tp.base + k == P.E - 1);
+          const float wsum = c.w[k] + c.wr;
+          float lam = 0.0f;
+          f3 t = zero3<float>();
+          if (on && wsum > 0.0f) project_edge<float>(epred[k] + (dxr - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+          R.S[k] += lam;
+          R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
+          back = axpy(back, lam * c.wr, t);
+          lamv[k] += lam;   // the closing edge's slot is idle in the red sweep
         }
         R.dx[0] -= shfl3(back, tp.pl);
-        (void)lam3;
       }
     }
     if (MODE >= 1 && lam_rows) store_row<VPL>(lam_rows + (size_t)it * P.NS, tp.base, P.NS, lamv);
