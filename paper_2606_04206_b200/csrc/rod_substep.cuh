@@ -394,6 +394,15 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
   return out;
 }
 
+// Eq.10 with compliance on one edge, loop invariants precomputed: idn = 1 / (w_j + w_j+1 + atil), or 0 for a slot
+// that is not projected (then lam = 0 and t is finite: the caller's updates change nothing).
+__device__ __forceinline__ void project_edge_pre(const f3& e, float l0, float atil, float S, float idn, float& lam, f3& t) {
+  const float L2 = fmaxf(dot(e, e), 1.0e-30f);   // a padding slot has e = 0: keep t finite there, lam * t must be 0
+  const float iL = rsqrt_(L2);
+  t = iL * e;
+  lam = ((L2 * iL - l0) - atil * S) * idn;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // One substep.  On entry `ec` holds the edge geometry of s.x (tangents, inverse lengths, previous lane's last
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
@@ -547,6 +556,19 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   }
   // -- A5 projection loop
   const float atil = c.stretch * inv_h * inv_h;
+  // loop invariants of Eq.10 per owned edge: inverse mass of its far vertex and 1 / (w_j + w_j+1 + atil), 0 for a
+  // slot that is not projected (padding, pinned at both ends).  The loop body is then branch-free; with division as
+  // MUFU.RCP x numerator (-prec-div=false) the multiplier has the same bits as dividing inside the loop.
+  float idn[VPL], wfar[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    const bool red = (k & 1) == 0;
+    const bool rem = !red && ((k == VPL - 1) || (k == tp.ks));
+    const bool on = red ? ((k + 1 < tp.nv) && tp.evalid[k]) : (tp.evalid[k] && (k <= tp.ks));
+    wfar[k] = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
+    const float wsum = c.w[k] + wfar[k];
+    idn[k] = (P.stretch_mode == 1 && on && wsum > 0.0f) ? 1.0f / (wsum + atil) : 0.0f;
+  }
   for (int it = 0; it < P.N_C; ++it) {
     float lamv[VPL];
 #pragma unroll
@@ -555,14 +577,12 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       // red: even slots, both end points local
 #pragma unroll
       for (int k = 0; k < VPL; k += 2) {
-        const bool on = (k + 1 < tp.nv) && tp.evalid[k];
-        const float wsum = c.w[k] + c.w[k + 1];
-        float lam = 0.0f;
-        f3 t = zero3<float>();
-        if (on && wsum > 0.0f) project_edge<float>(epred[k] + (R.dx[k + 1] - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+        float lam;
+        f3 t;
+        project_edge_pre(epred[k] + (R.dx[k + 1] - R.dx[k]), c.l0, atil, R.S[k], idn[k], lam, t);
         R.S[k] += lam;
         R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
-        R.dx[k + 1] = axpy(R.dx[k + 1], -lam * c.w[k + 1], t);
+        R.dx[k + 1] = axpy(R.dx[k + 1], -lam * wfar[k], t);
         lamv[k] = lam;
       }
       // black: odd slots; the lane's last slot crosses to slot 0 of the next lane
@@ -571,19 +591,20 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         f3 back = zero3<float>();
 #pragma unroll
         for (int k = 1; k < VPL; k += 2) {
-          const bool rem = (k == VPL - 1) || (k == tp.ks);
-          const bool on = tp.evalid[k] && (k <= tp.ks);
-          const float wn = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
-          const f3 dxn = rem ? dxr : R.dx[k + 1 < VPL ? k + 1 : k];
-          const float wsum = c.w[k] + wn;
-          float lam = 0.0f;
-          f3 t = zero3<float>();
-          if (on && wsum > 0.0f) project_edge<float>(epred[k] + (dxn - R.dx[k]), wsum, c.l0, atil, R.S[k], lam, t);
+          const bool last = (k == VPL - 1), rem = last || (k == tp.ks);
+          const f3 dxn = last ? dxr : (rem ? dxr : R.dx[k + 1 < VPL ? k + 1 : k]);
+          float lam;
+          f3 t;
+          project_edge_pre(epred[k] + (dxn - R.dx[k]), c.l0, atil, R.S[k], idn[k], lam, t);
           R.S[k] += lam;
           R.dx[k] = axpy(R.dx[k], lam * c.w[k], t);
-          if (rem) { if (on) back = (lam * wn) * t; }
-          else if (k + 1 < VPL) R.dx[k + 1] = axpy(R.dx[k + 1], -lam * wn, t);
-            lamv[k] = lam;
+          const float cn = lam * wfar[k];
+          if (last) back = axpy(back, cn, t);
+          else {   // at most one remote edge per lane is projected: `back` receives one non-zero term
+            back = axpy(back, rem ? cn : 0.0f, t);
+            R.dx[k + 1 < VPL ? k + 1 : k] = axpy(R.dx[k + 1 < VPL ? k + 1 : k], rem ? 0.0f : -cn, t);
+          }
+          lamv[k] = lam;
         }
         R.dx[0] -= shfl3(back, tp.pl);
       }

@@ -63,16 +63,11 @@ __device__ __forceinline__ float warp_sum(float v) {
 // shared-memory position of vertex i: natural order plus one pad word per 32, so that both access patterns are
 // bank-conflict free: the lanes' own vertices (stride VPL across lanes) and runs of consecutive vertices (candidates)
 template <int VPL> __device__ __forceinline__ int vpos(int i) { return i + (i >> 5); }
-__device__ __forceinline__ float warp_max(float v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(DLO_FULL, v, o));
-  return v;
-}
-__device__ __forceinline__ float warp_min(float v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(DLO_FULL, v, o));
-  return v;
-}
+// max / min over the warp of NON-NEGATIVE values (squared lengths): their bit patterns order like unsigned integers,
+// so one REDUX replaces five shuffle + compare rounds.  A NaN compares above every number: it survives a max (the
+// bounds built on it then fail, which is the conservative side) and is dropped by a min.
+__device__ __forceinline__ float warp_max(float v) { return __uint_as_float(__reduce_max_sync(DLO_FULL, __float_as_uint(v))); }
+__device__ __forceinline__ float warp_min(float v) { return __uint_as_float(__reduce_min_sync(DLO_FULL, __float_as_uint(v))); }
 __device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
 __device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
 
@@ -173,6 +168,11 @@ template <int VPL> __device__ __forceinline__ void load_env(const KParams& P, in
     c.w[k] = (tp.vvalid[k] && c.kin[k] == KIN_FREE) ? c.inv_m : 0.0f;
   }
   c.wr = shfl(c.w[0], tp.nl);
+  // opaque from here on: otherwise the compiler, short of registers, re-derives w[k] from kin[k], the lane index and N at
+  // every use inside the projection loop (4 instructions instead of a register or one reload)
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) asm volatile("" : "+f"(c.w[k]));
+  asm volatile("" : "+f"(c.wr));
 }
 
 // cached edge geometry of the CURRENT positions: unit tangent and inverse length per owned edge, plus the copy
