@@ -110,6 +110,9 @@ static void fill_params(const dlo_config& c, KParams& P) {
   P.G = c.n_grippers; P.M = P.G ? c.n_grasp_max : 1; P.K = c.n_primitives;
   P.cand_cap = round_up(4 * P.N, 32);
   P.list_margin = c.rope_radius;   // a quarter of the candidate distance 2(r_a+r_b)
+  P.vote_mode = 3;
+  if (const char* ov = getenv("DLO_LIST_MARGIN")) P.list_margin = c.rope_radius * (float)atof(ov);   // tuning overrides (no effect on results)
+  if (const char* ov = getenv("DLO_VOTE")) P.vote_mode = atoi(ov) & 3;
   P.h = c.dt / (float)c.n_substeps; P.inv_h = 1.0f / P.h;
   for (int k = 0; k < 3; ++k) P.g[k] = c.gravity[k];
   P.r = c.rope_radius; P.inv_eps = 1.0f / c.contact_softness; P.f_thresh = c.influence_threshold; P.e_rest = c.restitution;

@@ -23,6 +23,31 @@ __device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float w
   epb += eb;
 }
 
+// The same with the loop invariants precomputed (idn = 1 / (wk + wn + atil), 0 for a slot that is not projected) and no
+// branch: an idle slot has lam = 0 on the tape and idn = 0, so every update below adds a zero.
+__device__ __forceinline__ void edge_reverse_pre(const f3& epred, float lam, float wk, float wn, float idn, float atil, f3& dxk, f3& dxn, float& S,
+                                                 f3& gk, f3& gn, float& Sb, float& atilbar, f3& epb) {
+  const f3 ep = epred + (dxn - dxk);                // = (L - lam (wk+wn)) t
+  const float ep2 = fmaxf(dot(ep, ep), 1.0e-30f);   // (padding slots have ep = 0: keep t finite)
+  const float iLp = rsqrt_(ep2);
+  const f3 t = iLp * ep;
+  const float L = ep2 * iLp + lam * (wk + wn);
+  const float Spost = S;
+  S -= lam;
+  dxk = axpy(dxk, -lam * wk, t);
+  dxn = axpy(dxn, lam * wn, t);
+  // project_edge_adj (rod_adj.cuh) with the division by (wk + wn + atil) replaced by the stored reciprocal
+  const f3 g = wk * gk - wn * gn;
+  const float numbar = (dot(g, t) + Sb) * idn;
+  atilbar -= numbar * Spost;
+  Sb -= atil * numbar;
+  const f3 tbar = lam * g;
+  const f3 eb = numbar * t + (1.0f / L) * (tbar - dot(tbar, t) * t);
+  gn += eb;
+  gk -= eb;
+  epb += eb;
+}
+
 // Reverse of one substep.  s0 = state at its start (from the tape); A: in = adjoint of the state at its end,
 // out = adjoint of the state at its start.  G accumulates material / action adjoints of this lane.
 template <int VPL>
@@ -68,7 +93,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
     edge_refresh<VPL>(tp, s, ec);
     edge_prev_refresh<VPL>(tp, s, ec);
-    substep_idle_syncs(sm);
+    substep_idle_syncs(P, sm);
   }
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
 
@@ -195,6 +220,16 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
   const float atil = c.stretch * inv_h * inv_h;
   float atilbar = 0.0f;
+  float idn[VPL], wfar[VPL];   // as in substep(): far-vertex inverse mass, 1 / (w_j + w_j+1 + atil) or 0 for an idle slot
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) {
+    const bool red = (k & 1) == 0;
+    const bool rem = !red && ((k == VPL - 1) || (k == tp.ks));
+    const bool on = red ? ((k + 1 < tp.nv) && tp.evalid[k]) : (tp.evalid[k] && (k <= tp.ks));
+    wfar[k] = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
+    const float wsum = c.w[k] + wfar[k];
+    idn[k] = (P.stretch_mode == 1 && on && wsum > 0.0f) ? 1.0f / (wsum + atil) : 0.0f;
+  }
   for (int it = P.N_C - 1; it >= 0; --it) {
     float lamv[VPL];   // multipliers of this iteration, one per owned edge (the odd ring's closing edge sits in its idle red slot)
     load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it) * P.NS, tp.base, P.NS, lamv);
@@ -240,24 +275,23 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         const f3 dxr0 = dxr, gr0 = gr;
 #pragma unroll
         for (int k = 1; k < VPL; k += 2) {
-          const bool rem = (k == VPL - 1) || (k == tp.ks);
-          const bool on = tp.evalid[k] && (k <= tp.ks);
-          const float wn = rem ? c.wr : c.w[k + 1 < VPL ? k + 1 : k];
-          if (on && c.w[k] + wn > 0.0f) {
-            const float lam = lamv[k];
-            if (rem) edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
-            else edge_reverse(epred[k], lam, c.w[k], wn, atil, R.dx[k], R.dx[k + 1 < VPL ? k + 1 : k], R.S[k], dxb[k], dxb[k + 1 < VPL ? k + 1 : k], Sb[k], atilbar, epb[k]);
+          if (k == VPL - 1) {
+            edge_reverse_pre(epred[k], lamv[k], c.w[k], wfar[k], idn[k], atil, R.dx[k], dxr, R.S[k], dxb[k], gr, Sb[k], atilbar, epb[k]);
+          } else {   // the far vertex is remote when this is the lane's last valid slot
+            const int kn = k + 1 < VPL ? k + 1 : k;
+            const bool rem = (k == tp.ks);
+            f3 dxn = rem ? dxr : R.dx[kn], gn = rem ? gr : dxb[kn];
+            edge_reverse_pre(epred[k], lamv[k], c.w[k], wfar[k], idn[k], atil, R.dx[k], dxn, R.S[k], dxb[k], gn, Sb[k], atilbar, epb[k]);
+            dxr = rem ? dxn : dxr; gr = rem ? gn : gr;
+            R.dx[kn] = rem ? R.dx[kn] : dxn; dxb[kn] = rem ? dxb[kn] : gn;
           }
         }
         R.dx[0] += shfl3(dxr - dxr0, tp.pl);
         dxb[0] += shfl3(gr - gr0, tp.pl);
       }
 #pragma unroll
-      for (int k = 0; k < VPL; k += 2) {   // red
-        const bool on = (k + 1 < tp.nv) && tp.evalid[k];
-        if (on && c.w[k] + c.w[k + 1] > 0.0f)
-          edge_reverse(epred[k], lamv[k], c.w[k], c.w[k + 1], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
-      }
+      for (int k = 0; k < VPL; k += 2)   // red
+        edge_reverse_pre(epred[k], lamv[k], c.w[k], wfar[k], idn[k], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
     }
   }
   G.gm[GM_STRETCH] += (P.stretch_mode == 1) ? atilbar * inv_h * inv_h : 0.0f;

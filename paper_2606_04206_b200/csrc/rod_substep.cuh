@@ -407,9 +407,9 @@ __device__ __forceinline__ void project_edge_pre(const f3& e, float l0, float at
 // One substep.  On entry `ec` holds the edge geometry of s.x (tangents, inverse lengths, previous lane's last
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
 // the barriers of substep() for a warp that skips the recompute (it must still take part in them, votes included)
-__device__ __forceinline__ void substep_idle_syncs(const WarpSmem& sm) {
+__device__ __forceinline__ void substep_idle_syncs(const KParams& P, const WarpSmem& sm) {
   phase_sync(sm);
-  if (phase_vote(sm, false)) phase_vote(sm, false);
+  if ((P.vote_mode & 1) && phase_vote(sm, false) && (P.vote_mode & 2)) phase_vote(sm, false);
   phase_sync(sm);
   phase_sync(sm);
 }
@@ -477,9 +477,11 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   }
   auto build_list = [&](bool vote) {
     // is the pair list still a superset?  (no vertex further than list_margin from where it was built)
-    bool fresh = cc.nlist < 0, overflow = false;
+    // (a list that was truncated is rebuilt at every use: that is this env's own business, the vote is about movement only)
+    const bool trunc = cc.nlist < 0;
+    bool fresh = false, overflow = false;
     int nuse = cc.nlist;
-    if (!fresh) {
+    if (!trunc) {
       float m2 = 0.0f;
 #pragma unroll
       for (int k = 0; k < VPL; ++k)
@@ -488,7 +490,8 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       const float wm = warp_max(m2);
       fresh = !(wm <= lm * lm);
     }
-    if (vote) fresh = phase_vote(sm, fresh) || fresh;   // a warp of the CTA rebuilds: all do (they would wait for it anyway)
+    if (vote && (P.vote_mode & 2)) fresh = phase_vote(sm, fresh);   // a warp of the CTA rebuilds: all do (they would wait for it anyway)
+    fresh = fresh || trunc;
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
       const int i = vpos<VPL>(tp.base + k);
@@ -548,8 +551,9 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   {
     const float need = 2.0f * P.r + 1.0e-6f;
     const bool want = P.self_contact && !(cc.dref - 2.0f * D1 >= need);
-    if (phase_vote(sm, want) && P.self_contact) {
-      build_list(true);
+    const bool go = (P.vote_mode & 1) ? phase_vote(sm, want) : want;
+    if (go && P.self_contact) {
+      build_list((P.vote_mode & 1) != 0);
       built = true;
       D1 = 0.0f;
     }

@@ -28,6 +28,7 @@ struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
   int G, M, K, cand_cap;
   float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
+  int vote_mode;         // bit 0: the warps of a CTA refresh their contact data together; bit 1: ... and rebuild their pair lists together
   float list_margin;     // the self-contact pair list stays valid while no vertex has moved further than this since it was built
   int prim_type[16];
   const float* mat;      // [B][MAT_N]
