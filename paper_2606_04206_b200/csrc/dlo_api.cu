@@ -65,11 +65,12 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
   P.sm_prim = take(P.K * PRIM_SM_STRIDE);
   P.sm_q = take(P.G * P.M * 3);
   P.sm_ys = P.sm_acc = P.sm_vs = P.sm_mid = P.sm_dp = P.sm_cand = 0;
-  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = P.sm_blk = P.sm_xref = 0;
+  P.sm_lam = P.sm_dpbar = P.sm_ybar = P.sm_vbar = P.sm_posebar = P.sm_blk = P.sm_xref = P.sm_hot = 0;
   if (P.self_contact) {
     P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
     P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap);   // candidates + prefilter survivors (ushort each)
     P.sm_blk = take(4 * 32);
+    P.sm_hot = take(P.hot_cap / 2);   // near pairs (ushort each), kept across substeps
     if (!adjoint) P.sm_xref = take(3 * NP);   // positions at which the pair list was built (must outlive the substep)
   }
   if (adjoint) {
@@ -109,6 +110,7 @@ static void fill_params(const dlo_config& c, KParams& P) {
   P.self_contact = c.enable_self_contact != 0; P.self_skip = c.self_skip;
   P.G = c.n_grippers; P.M = P.G ? c.n_grasp_max : 1; P.K = c.n_primitives;
   P.cand_cap = round_up(4 * P.N, 32);
+  P.hot_cap = 32 * vpl_for(P.N);   // <= a third of the 3 x 33 VPL floats of sm.vs, which holds two such arrays during a mid-loop rebuild
   P.list_margin = c.rope_radius;   // a quarter of the candidate distance 2(r_a+r_b)
   P.vote_mode = 3;
   if (const char* ov = getenv("DLO_LIST_MARGIN")) P.list_margin = c.rope_radius * (float)atof(ov);   // tuning overrides (no effect on results)

@@ -290,8 +290,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         dxb[0] += shfl3(gr - gr0, tp.pl);
       }
 #pragma unroll
-      for (int k = 0; k < VPL; k += 2)   // red
-        edge_reverse_pre(epred[k], lamv[k], c.w[k], wfar[k], idn[k], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
+      for (int k = 0; k < VPL; k += 2)   // red (an odd ring keeps the closing edge's multiplier in its idle red slot: not this edge's)
+        edge_reverse_pre(epred[k], idn[k] != 0.0f ? lamv[k] : 0.0f, c.w[k], wfar[k], idn[k], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
     }
   }
   G.gm[GM_STRETCH] += (P.stretch_mode == 1) ? atilbar * inv_h * inv_h : 0.0f;

@@ -9,12 +9,14 @@ namespace dlo {
 struct WarpSmem {
   float *pose, *prim, *q, *ys, *acc, *vs, *mid, *dp, *lam, *dpbar, *ybar, *vbar, *posebar, *blk, *xref;
   unsigned short* cand;
+  unsigned short* hot;   // near pairs of the last full filter (in pair order), kept across substeps
   float* base;        // the warp's shared-memory block (non-inlined helpers rebuild the view from this one pointer)
   int sync_threads;   // > 0: warps of the CTA walk the phases in lockstep (named barrier over this many threads)
   int NP;   // row stride of the per-vertex arrays: 33*VPL (32*VPL vertices + pad words, see vpos)
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
     pose = base + P.sm_pose; prim = base + P.sm_prim; q = base + P.sm_q; ys = base + P.sm_ys; acc = base + P.sm_acc;
     vs = base + P.sm_vs; mid = base + P.sm_mid; dp = base + P.sm_dp; cand = reinterpret_cast<unsigned short*>(base + P.sm_cand);
+    hot = reinterpret_cast<unsigned short*>(base + P.sm_hot);
     lam = base + P.sm_lam; dpbar = base + P.sm_dpbar; ybar = base + P.sm_ybar; vbar = base + P.sm_vbar; posebar = base + P.sm_posebar; blk = base + P.sm_blk; xref = base + P.sm_xref;
     NP = np;
     this->base = base;
@@ -42,13 +44,15 @@ __device__ __forceinline__ bool phase_vote(const WarpSmem& sm, bool v) {
 // the exact minimum pair distance there (dref < 0: nothing known, build at first need; huge: never build)
 template <int VPL> struct ContactCache {
   f3 xref[VPL];
-  float dref;
+  float dref;  // minimum distance, at xref, over the pairs that are NOT in the near list
   int nlist;   // size of the pair list in shared memory (build_pair_list); < 0: none yet or truncated, rebuild at next use
+  int nhot;    // size of the near list (sm.hot); < 0: none (then dref covers every pair)
   __device__ __forceinline__ void reset(float d) {
 #pragma unroll
     for (int k = 0; k < VPL; ++k) xref[k] = zero3<float>();
     dref = d;
     nlist = -1;
+    nhot = -1;
   }
 };
 
@@ -209,23 +213,68 @@ __device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* s
   return nsurv;   // > cand_cap: truncated
 }
 
-// exact narrow phase at x^p (in sm.ys) over the pair list, ordered compaction into the candidate list
-struct CandOut { int ncand; float dmin; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b)
+// exact narrow phase at x^p (in sm.ys) over the pair list, ordered compaction into the candidate list.  The same pass
+// splits the pairs into NEAR (closer than 3 r_sum / 2, kept in sm.hot in pair order) and FAR: between full filters
+// only the near pairs are measured again (filter_near, every substep), the far ones are covered by the Lipschitz
+// bound on dfar.  Too many near pairs for sm.hot: no near list (nhot = -1), dfar covers every pair.
+struct CandOut { int ncand, nhot; float dmin, dfar; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b); dfar: over the far ones
 template <int VPL>
 __device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, float* smbase, int nsurv, bool overflow) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int N = P.N, NP = sm.NP;
   const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
+  const float near2 = 9.0f * P.r * P.r;
   const unsigned short* surv = sm.cand + P.cand_cap;
-  int ncand = 0;
-  float d2min = lim * lim;
+  int ncand = 0, nhot = 0;
+  float d2min = lim * lim, d2far = lim * lim;
   for (int p0 = 0; p0 < nsurv; p0 += 32) {
     const int p = p0 + lane;
-    bool hit = false;
+    bool hit = false, near = false;
     unsigned c = 0u;
     if (p < nsurv) {
       c = surv[p];
+      const int a = c >> 8, b = c & 255, an = (a + 1 < N) ? a + 1 : 0, bn = (b + 1 < N) ? b + 1 : 0;
+      const float d2 = pair_dist2(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn));
+      hit = d2 < lim * lim;
+      near = d2 < near2;
+      d2min = fminf(d2min, d2);
+      if (!near) d2far = fminf(d2far, d2);
+    }
+    const unsigned m = __ballot_sync(DLO_FULL, hit), mh = __ballot_sync(DLO_FULL, near);
+    if (hit) sm.cand[ncand + __popc(m & ((1u << lane) - 1u))] = (unsigned short)c;
+    if (near) {
+      const int pos = nhot + __popc(mh & ((1u << lane) - 1u));
+      if (pos < P.hot_cap) sm.hot[pos] = (unsigned short)c;
+    }
+    ncand += __popc(m);
+    nhot += __popc(mh);
+  }
+  __syncwarp();
+  CandOut out;
+  out.ncand = ncand;
+  out.dmin = overflow ? 0.0f : sqrt_(warp_min(d2min));
+  const bool nolist = overflow || nhot > P.hot_cap;
+  out.nhot = nolist ? -1 : nhot;
+  out.dfar = nolist ? out.dmin : sqrt_(warp_min(d2far));
+  return out;
+}
+
+// the near pairs measured again at x^p (in sm.ys): candidate list = those closer than 2(r_a+r_b), in pair order
+template <int VPL>
+__device__ __noinline__ CandOut filter_near(const KParams& P, int lane, float* smbase, int nhot) {
+  WarpSmem sm;
+  sm.init(P, smbase, 33 * VPL);
+  const int N = P.N, NP = sm.NP;
+  const float lim = 4.0f * P.r;
+  int ncand = 0;
+  float d2min = lim * lim;
+  for (int p0 = 0; p0 < nhot; p0 += 32) {
+    const int p = p0 + lane;
+    bool hit = false;
+    unsigned c = 0u;
+    if (p < nhot) {
+      c = sm.hot[p];
       const int a = c >> 8, b = c & 255, an = (a + 1 < N) ? a + 1 : 0, bn = (b + 1 < N) ? b + 1 : 0;
       const float d2 = pair_dist2(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn));
       hit = d2 < lim * lim;
@@ -237,8 +286,9 @@ __device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, fl
   }
   __syncwarp();
   CandOut out;
-  out.ncand = ncand;
-  out.dmin = overflow ? 0.0f : sqrt_(warp_min(d2min));
+  out.ncand = ncand; out.nhot = nhot;
+  out.dmin = sqrt_(warp_min(d2min));
+  out.dfar = 0.0f;
   return out;
 }
 
@@ -461,13 +511,17 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
 
   // Self-contact is evaluated lazily (exactly): segment distance is 1-Lipschitz in the end points, so with d_ref the
-  // minimum pair distance at the positions x_ref where the candidate list was last built, no pair can penetrate
-  // while d_ref - 2 (max_i |x^p_i - x_ref,i| + max_i |dx_i|) >= r_a + r_b.  Only when that bound fails is the list
-  // (re)built at x^p and the Jacobi pass run.  A pass that cannot apply a correction changes nothing, so the
-  // state is identical to building and sweeping every time.
+  // minimum distance of a set of pairs at the positions x_ref where they were last measured, none of them can
+  // penetrate while d_ref - 2 (max_i |x^p_i - x_ref,i| + max_i |dx_i|) >= r_a + r_b.  A full filter (pair list at
+  // x^p, every pair measured) splits the pairs into near ones (closer than 3/2 r_sum, a handful: real contacts
+  // and sharp folds) and far ones.  The far ones are covered by that bound with d_ref = their minimum distance, which
+  // leaves r_sum / 2 of slack: a full filter every few tens of substeps.  The near ones are measured again at every
+  // x^p (filter_near) and swept when they can penetrate within the iteration's max |dx|.  A pass that cannot apply a
+  // correction changes nothing, so the state is identical to building the whole list and sweeping it every time.
   R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
   bool built = false;
   float D1 = 0.0f;
+  float dnear = 1.0e30f;   // exact minimum distance at x^p over the pairs of the candidate list in use
   if (P.self_contact) {
     float m2 = 0.0f;
 #pragma unroll
@@ -537,12 +591,26 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       }
     }
     __syncwarp();
+    // a rebuild in the middle of the projection loop, after sweeps over the near pairs have applied corrections: their
+    // depth sums D_p move to the pairs' positions in the new list (sm.vs is free until the friction pass)
+    const int nold = R.any_pen ? R.ncand : 0;
+    unsigned* oldc = reinterpret_cast<unsigned*>(sm.vs);
+    float* oldd = sm.vs + P.hot_cap;
+    for (int p = tp.lane; p < nold; p += 32) { oldc[p] = sm.cand[p]; oldd[p] = sm.dp[p]; }
+    __syncwarp();
     const CandOut co = filter_candidates<VPL>(P, tp.lane, sm.base, nuse, overflow);
     R.ncand = co.ncand;
-    cc.dref = co.dmin;
+    cc.dref = co.dfar;
+    cc.nhot = co.nhot;
+    dnear = co.dmin;
 #pragma unroll
     for (int k = 0; k < VPL; ++k) cc.xref[k] = R.xp[k];
-    for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
+    for (int p = tp.lane; p < R.ncand; p += 32) {
+      float d = 0.0f;
+      const unsigned code = sm.cand[p];
+      for (int q = 0; q < nold; ++q) if (oldc[q] == code) d = oldd[q];
+      sm.dp[p] = d;
+    }
     __syncwarp();
   };
 
@@ -556,6 +624,16 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       build_list((P.vote_mode & 1) != 0);
       built = true;
       D1 = 0.0f;
+    } else if (P.self_contact && cc.nhot > 0) {
+      // the far pairs are safe where they are: measure the near ones at x^p, they are this substep's candidates
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k]);
+      __syncwarp();
+      const CandOut co = filter_near<VPL>(P, tp.lane, sm.base, cc.nhot);
+      R.ncand = co.ncand;
+      dnear = co.dmin;
+      for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
+      __syncwarp();
     }
   }
   // -- A5 projection loop
@@ -640,13 +718,14 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
 #pragma unroll
       for (int k = 0; k < VPL; ++k) m2 = fmaxf(m2, dot(R.dx[k], R.dx[k]));
       const float Dm = sqrt_(warp_max(m2)), need = 2.0f * P.r + 1.0e-6f;
-      sweep = !(cc.dref - 2.0f * (D1 + Dm) >= need);
-      if (sweep && !built) {
+      bool far_unsafe = !(cc.dref - 2.0f * (D1 + Dm) >= need);
+      if (far_unsafe && !built) {
         build_list(false);
         built = true;
         D1 = 0.0f;
-        sweep = !(cc.dref - 2.0f * Dm >= need);
+        far_unsafe = !(cc.dref - 2.0f * Dm >= need);
       }
+      sweep = far_unsafe || !(dnear - 2.0f * Dm >= need);
     }
     if (sweep && R.ncand > 0) {
 #pragma unroll

@@ -26,7 +26,7 @@ enum { PRIM_NP = 10, PRIM_SM_STRIDE = 20, PRIM_BC = 16, PRIM_BR = 19 };
 
 struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
-  int G, M, K, cand_cap;
+  int G, M, K, cand_cap, hot_cap;
   float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
   int vote_mode;         // bit 0: the warps of a CTA refresh their contact data together; bit 1: ... and rebuild their pair lists together
   float list_margin;     // the self-contact pair list stays valid while no vertex has moved further than this since it was built
@@ -48,7 +48,7 @@ struct KParams {
   float* g_actions;      // [H][B][G][6] (may be null)
   uint8_t* tape_flag;    // [stride*n_sub][B]: 1 if the substep applied a self-contact correction (written by the replay)
   // per-warp shared memory layout (float offsets from the warp's base), set by the host
-  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_blk, sm_xref, sm_warp_floats;
+  int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_blk, sm_xref, sm_hot, sm_warp_floats;
 };
 
 // per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
