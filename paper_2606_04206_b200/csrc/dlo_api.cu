@@ -113,6 +113,8 @@ static void fill_params(const dlo_config& c, KParams& P) {
   P.hot_cap = 32 * vpl_for(P.N);   // <= a third of the 3 x 33 VPL floats of sm.vs, which holds two such arrays during a mid-loop rebuild
   P.list_margin = c.rope_radius;   // a quarter of the candidate distance 2(r_a+r_b)
   P.vote_mode = 3;
+  P.near_dist = 3.0f * c.rope_radius;   // 3/2 (r_a + r_b): half of (r_a + r_b) of slack for the far pairs
+  if (const char* ov = getenv("DLO_NEAR")) P.near_dist = c.rope_radius * (float)atof(ov);   // 0: no near list
   if (const char* ov = getenv("DLO_LIST_MARGIN")) P.list_margin = c.rope_radius * (float)atof(ov);   // tuning overrides (no effect on results)
   if (const char* ov = getenv("DLO_VOTE")) P.vote_mode = atoi(ov) & 3;
   P.h = c.dt / (float)c.n_substeps; P.inv_h = 1.0f / P.h;

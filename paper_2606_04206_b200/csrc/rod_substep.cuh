@@ -224,7 +224,7 @@ __device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, fl
   sm.init(P, smbase, 33 * VPL);
   const int N = P.N, NP = sm.NP;
   const float lim = 4.0f * P.r;   // 2 (r_a + r_b)
-  const float near2 = 9.0f * P.r * P.r;
+  const float near2 = P.near_dist * P.near_dist;
   const unsigned short* surv = sm.cand + P.cand_cap;
   int ncand = 0, nhot = 0;
   float d2min = lim * lim, d2far = lim * lim;

@@ -29,6 +29,7 @@ struct KParams {
   int G, M, K, cand_cap, hot_cap;
   float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
   int vote_mode;         // bit 0: the warps of a CTA refresh their contact data together; bit 1: ... and rebuild their pair lists together
+  float near_dist;       // pairs closer than this at a full filter go to the near list (measured every substep)
   float list_margin;     // the self-contact pair list stays valid while no vertex has moved further than this since it was built
   int prim_type[16];
   const float* mat;      // [B][MAT_N]
