@@ -41,6 +41,10 @@ struct dlo_sim {
   cudaStream_t aux = nullptr;
   cudaEvent_t ev_fwd = nullptr, ev_rep[2] = {nullptr, nullptr}, ev_adj[2] = {nullptr, nullptr};
   int *grasp = nullptr, *flags = nullptr;
+  // env -> warp-slot order (k_sort_envs): work statistics of the last forward chunk / of the tape in each tape buffer, the orders made from them
+  int *stat = nullptr, *stat_rep[2] = {nullptr, nullptr}, *perm_main = nullptr, *perm_rep = nullptr;
+  bool stat_valid = false, stat_rep_valid[2] = {false, false};
+  int chunk = 100;                 // frames per forward launch when re-ordering is on (0: one launch, identity order)
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
   int H_actions = 0, H_done = 0, stride = 0;
@@ -207,6 +211,10 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   CUD(dalloc(&s->state, B * s->blk));
   CUD(dalloc(&s->state0, B * s->blk));
   CUD(dalloc(&s->flags, B));
+  CUD(dalloc(&s->stat, 2 * B)); CUD(dalloc(&s->stat_rep[0], 2 * B)); CUD(dalloc(&s->stat_rep[1], 2 * B));
+  CUD(dalloc(&s->perm_main, B)); CUD(dalloc(&s->perm_rep, B));
+  if (!P.self_contact) s->chunk = 0;   // the order only matters for the self-contact work
+  if (const char* ov = getenv("DLO_CHUNK")) s->chunk = std::max(0, atoi(ov));   // tuning override (no effect on results)
   CUD(cudaMemsetAsync(s->flags, 0, B * sizeof(int), s->stream));
   CUD(cudaMemsetAsync(s->pins, 0, B * P.N, s->stream));
   CUD(cudaMemsetAsync(s->grasp, 0xff, B * P.G * P.M * sizeof(int), s->stream));
@@ -231,7 +239,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2};
+                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
   for (void* p : dev) if (p) cudaFree(p);
   if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
   for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
@@ -334,6 +342,32 @@ static cudaError_t launch_forward(dlo_sim* s, KParams P, int t0, int t1, int str
 #undef DLO_FWD_CASE
 }
 
+static cudaError_t sort_envs(dlo_sim* s, const int* stat, int col, int shift, int* perm, cudaStream_t st) {
+  k_sort_envs<<<1, 1024, 0, st>>>(s->P.B, stat, col, shift, perm);
+  s->launches += 1;
+  return cudaGetLastError();
+}
+// frames [t0, t1) of the plain forward rollout in launches of s->chunk frames; from the second launch on the envs are
+// taken in the order of the self-contact work they did in the launch before (heaviest first, like with like)
+static cudaError_t forward_chunks(dlo_sim* s, int t0, int t1, int stride) {
+  for (int a = t0; a < t1;) {
+    const int b = (s->chunk > 0 && a + s->chunk < t1) ? a + s->chunk : t1;
+    KParams Pc = s->P;
+    Pc.stat = s->chunk > 0 ? s->stat : nullptr;
+    Pc.perm = nullptr;
+    if (s->chunk > 0 && s->stat_valid) {
+      cudaError_t e = sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream);
+      if (e != cudaSuccess) return e;
+      Pc.perm = s->perm_main;
+    }
+    cudaError_t e = launch_forward(s, Pc, a, b, stride, false, s->stream);
+    if (e != cudaSuccess) return e;
+    s->stat_valid = s->chunk > 0;
+    a = b;
+  }
+  return cudaSuccess;
+}
+
 // tape buffers of one checkpoint segment (two when there are several segments and memory allows: DESIGN.md section 5)
 static dlo_status ensure_tape(dlo_sim* s, int H, int stride) {
   const int B = s->P.B;
@@ -382,19 +416,26 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
   }
   s->tape_seg = -1;
+  s->stat_valid = s->stat_rep_valid[0] = s->stat_rep_valid[1] = false;
   if (horizon > 0 && stride > 0) {
     // the last segment is run in tape mode, so that the reverse pass can start without replaying it
     dlo_status st = ensure_tape(s, horizon, stride);
     if (st) return st;
     const int nseg = (horizon + stride - 1) / stride, t_last = (nseg - 1) * stride;
     const bool two = nseg > 1 && s->tape2 && s->tape_flag2;
-    if (t_last > 0) CU(launch_forward(s, s->P, 0, t_last, stride, false, s->stream));
+    if (t_last > 0) CU(forward_chunks(s, 0, t_last, stride));
     KParams Pf = s->P;
-    Pf.tape = (two && ((nseg - 1) & 1)) ? s->tape2 : s->tape;
-    Pf.tape_flag = (two && ((nseg - 1) & 1)) ? s->tape_flag2 : s->tape_flag;
+    const int buf = (two && ((nseg - 1) & 1)) ? 1 : 0;
+    Pf.tape = buf ? s->tape2 : s->tape;
+    Pf.tape_flag = buf ? s->tape_flag2 : s->tape_flag;
+    if (s->chunk > 0) {
+      Pf.stat = s->stat_rep[buf];
+      if (s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }
+    }
     CU(launch_forward(s, Pf, t_last, horizon, stride, true, s->stream));
+    s->stat_rep_valid[buf] = s->chunk > 0;
     s->tape_seg = nseg - 1;
-  } else if (horizon > 0) CU(launch_forward(s, s->P, 0, horizon, stride, false, s->stream));
+  } else if (horizon > 0) CU(forward_chunks(s, 0, horizon, stride));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;
 }

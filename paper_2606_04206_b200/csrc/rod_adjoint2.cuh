@@ -402,8 +402,9 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 template <int VPL>
 __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_constant__ KParams P, int t0, int t1) {
   extern __shared__ __align__(16) float smem[];
-  const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
-  if (env >= P.B) return;
+  const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, slot = blockIdx.x * wpb + wib;
+  if (slot >= P.B) return;
+  const int env = P.perm ? P.perm[slot] : slot;
   WarpSmem sm;
   sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
   sm.sync_threads = 32 * min(wpb, P.B - (int)blockIdx.x * wpb);

@@ -163,6 +163,24 @@ __device__ __forceinline__ void load_actions(const KParams& P, int env, int lane
   }
 }
 
+// Env -> warp-slot order of the next launch: envs sorted by a work key, heaviest first (counting sort, one CTA).  The
+// warps of a CTA walk in lockstep and wait for their slowest member at every phase barrier, so envs that do the same
+// amount of self-contact work belong in the same CTA; envs are independent, the order changes no result.
+__global__ void __launch_bounds__(1024, 1) k_sort_envs(int B, const int* __restrict__ stat, int col, int shift, int* __restrict__ perm) {
+  __shared__ int hist[1024];
+  const int tid = threadIdx.x;
+  hist[tid] = 0;
+  __syncthreads();
+  for (int i = tid; i < B; i += 1024) atomicAdd(&hist[min(max(stat[2 * i + col] >> shift, 0), 1023)], 1);
+  __syncthreads();
+  if (tid == 0) {   // start offsets, descending keys
+    int run = 0;
+    for (int k = 1023; k >= 0; --k) { const int n = hist[k]; hist[k] = run; run += n; }
+  }
+  __syncthreads();
+  for (int i = tid; i < B; i += 1024) perm[atomicAdd(&hist[min(max(stat[2 * i + col] >> shift, 0), 1023)], 1)] = i;
+}
+
 template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<VPL>& s) {
   float a = 0.0f;
 #pragma unroll
@@ -205,8 +223,9 @@ template <int VPL> __device__ __forceinline__ void load_rows3(const float* __res
 template <int VPL, bool TAPE>
 __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forward(const __grid_constant__ KParams P, int t0, int t1, int stride) {
   extern __shared__ __align__(16) float smem[];
-  const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, env = blockIdx.x * wpb + wib;
-  if (env >= P.B) return;
+  const int wpb = blockDim.x >> 5, wib = threadIdx.x >> 5, slot = blockIdx.x * wpb + wib;
+  if (slot >= P.B) return;
+  const int env = P.perm ? P.perm[slot] : slot;
   WarpSmem sm;
   sm.init(P, smem + (size_t)wib * P.sm_warp_floats, 33 * VPL);
   sm.sync_threads = 32 * min(wpb, P.B - (int)blockIdx.x * wpb);
@@ -215,6 +234,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
   EnvConst<VPL> c;
   load_env<VPL>(P, env, tp, c);
   warp_setup<VPL>(P, env, tp.lane, sm);
+  int work = 0, npen = 0;
   const size_t blk = (size_t)STATE_ROWS * P.NS, rec = (size_t)tape_rows(P.N_C) * P.NS;
   LaneState<VPL> s;
   load_state<VPL>(P.state + (size_t)env * blk, tp.base, P.NS, s);
@@ -245,11 +265,13 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
       } else {
         substep<VPL, 0>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
       }
+      work += R.work; npen += R.any_pen;
     }
     if (stride > 0 && (t + 1) % stride == 0) store_state<VPL>(P.ckpt + ((size_t)((t + 1) / stride) * P.B + env) * blk, tp.base, P.NS, s);
   }
   if (TAPE) store_state<VPL>(P.tape + ((size_t)(t1 - t0) * P.n_sub * P.B + env) * rec, tp.base, P.NS, s);
   store_state<VPL>(P.state + (size_t)env * blk, tp.base, P.NS, s);
+  if (P.stat && tp.lane == 0) { P.stat[2 * env] = work; P.stat[2 * env + 1] = npen; }
   const bool ok = state_finite<VPL>(s);
   if (__any_sync(DLO_FULL, !ok) && tp.lane == 0) atomicOr(P.flags + env, FLAG_NONFINITE);
 }

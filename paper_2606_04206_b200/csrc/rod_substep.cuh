@@ -62,6 +62,7 @@ template <int VPL> struct SubRec {
   float S[VPL];
   unsigned active[VPL];   // bit k<K: primitive k responded; bit K+2g+f: finger f of gripper g responded
   int ncand, any_pen;
+  int work;               // rough count of the self-contact work this substep did (scheduling hint only)
   unsigned jac_mask;      // bit it: the Jacobi pass of iteration it applied at least one correction
 };
 
@@ -518,7 +519,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // leaves r_sum / 2 of slack: a full filter every few tens of substeps.  The near ones are measured again at every
   // x^p (filter_near) and swept when they can penetrate within the iteration's max |dx|.  A pass that cannot apply a
   // correction changes nothing, so the state is identical to building the whole list and sweeping it every time.
-  R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
+  R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u; R.work = 0;
   bool built = false;
   float D1 = 0.0f;
   float dnear = 1.0e30f;   // exact minimum distance at x^p over the pairs of the candidate list in use
@@ -599,6 +600,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     for (int p = tp.lane; p < nold; p += 32) { oldc[p] = sm.cand[p]; oldd[p] = sm.dp[p]; }
     __syncwarp();
     const CandOut co = filter_candidates<VPL>(P, tp.lane, sm.base, nuse, overflow);
+    R.work += fresh ? 24 : 8;
     R.ncand = co.ncand;
     cc.dref = co.dfar;
     cc.nhot = co.nhot;
@@ -630,6 +632,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k]);
       __syncwarp();
       const CandOut co = filter_near<VPL>(P, tp.lane, sm.base, cc.nhot);
+      R.work += 1;
       R.ncand = co.ncand;
       dnear = co.dmin;
       for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = 0.0f;
@@ -732,6 +735,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]);
       __syncwarp();
       const bool any = contact_pass<VPL>(P, tp.lane, sm.base, R.ncand);
+      R.work += any ? 3 : 1;
       __syncwarp();
       if (any) {
         R.any_pen = 1;
