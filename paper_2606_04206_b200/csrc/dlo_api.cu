@@ -44,7 +44,8 @@ struct dlo_sim {
   // env -> warp-slot order (k_sort_envs): work statistics of the last forward chunk / of the tape in each tape buffer, the orders made from them
   int *stat = nullptr, *stat_rep[2] = {nullptr, nullptr}, *perm_main = nullptr, *perm_rep = nullptr;
   bool stat_valid = false, stat_rep_valid[2] = {false, false};
-  int chunk = 100;                 // frames per forward launch when re-ordering is on (0: one launch, identity order)
+  int chunk = 100;                 // frames per forward launch when the forward re-orders (sort_mode bit 0)
+  int sort_mode = 6;               // bit 0: forward launches, bit 1: replays, bit 2: adjoint launches take the envs in sorted order
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
   int H_actions = 0, H_done = 0, stride = 0;
@@ -213,8 +214,9 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   CUD(dalloc(&s->flags, B));
   CUD(dalloc(&s->stat, 2 * B)); CUD(dalloc(&s->stat_rep[0], 2 * B)); CUD(dalloc(&s->stat_rep[1], 2 * B));
   CUD(dalloc(&s->perm_main, B)); CUD(dalloc(&s->perm_rep, B));
-  if (!P.self_contact) s->chunk = 0;   // the order only matters for the self-contact work
-  if (const char* ov = getenv("DLO_CHUNK")) s->chunk = std::max(0, atoi(ov));   // tuning override (no effect on results)
+  if (const char* ov = getenv("DLO_CHUNK")) s->chunk = std::max(1, atoi(ov));   // tuning overrides (no effect on results)
+  if (const char* ov = getenv("DLO_SORT")) s->sort_mode = atoi(ov) & 7;
+  if (!P.self_contact) s->sort_mode = 0;   // the order only matters for the self-contact work
   CUD(cudaMemsetAsync(s->flags, 0, B * sizeof(int), s->stream));
   CUD(cudaMemsetAsync(s->pins, 0, B * P.N, s->stream));
   CUD(cudaMemsetAsync(s->grasp, 0xff, B * P.G * P.M * sizeof(int), s->stream));
@@ -347,22 +349,24 @@ static cudaError_t sort_envs(dlo_sim* s, const int* stat, int col, int shift, in
   s->launches += 1;
   return cudaGetLastError();
 }
-// frames [t0, t1) of the plain forward rollout in launches of s->chunk frames; from the second launch on the envs are
-// taken in the order of the self-contact work they did in the launch before (heaviest first, like with like)
+// frames [t0, t1) of the plain forward rollout.  With sort_mode bit 0: in launches of s->chunk frames, from the second on
+// with the envs in the order of the self-contact work they did in the launch before (measured: no gain for the forward,
+// whose waiting warps leave their issue slots to the SM's other CTA; off by default)
 static cudaError_t forward_chunks(dlo_sim* s, int t0, int t1, int stride) {
+  const bool on = (s->sort_mode & 1) != 0;
   for (int a = t0; a < t1;) {
-    const int b = (s->chunk > 0 && a + s->chunk < t1) ? a + s->chunk : t1;
+    const int b = (on && a + s->chunk < t1) ? a + s->chunk : t1;
     KParams Pc = s->P;
-    Pc.stat = s->chunk > 0 ? s->stat : nullptr;
+    Pc.stat = on ? s->stat : nullptr;
     Pc.perm = nullptr;
-    if (s->chunk > 0 && s->stat_valid) {
+    if (on && s->stat_valid) {
       cudaError_t e = sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream);
       if (e != cudaSuccess) return e;
       Pc.perm = s->perm_main;
     }
     cudaError_t e = launch_forward(s, Pc, a, b, stride, false, s->stream);
     if (e != cudaSuccess) return e;
-    s->stat_valid = s->chunk > 0;
+    s->stat_valid = on;
     a = b;
   }
   return cudaSuccess;
@@ -428,12 +432,12 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     const int buf = (two && ((nseg - 1) & 1)) ? 1 : 0;
     Pf.tape = buf ? s->tape2 : s->tape;
     Pf.tape_flag = buf ? s->tape_flag2 : s->tape_flag;
-    if (s->chunk > 0) {
+    if (s->sort_mode) {
       Pf.stat = s->stat_rep[buf];
-      if (s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }
+      if ((s->sort_mode & 1) && s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }
     }
     CU(launch_forward(s, Pf, t_last, horizon, stride, true, s->stream));
-    s->stat_rep_valid[buf] = s->chunk > 0;
+    s->stat_rep_valid[buf] = s->sort_mode != 0;
     s->tape_seg = nseg - 1;
   } else if (horizon > 0) CU(forward_chunks(s, 0, horizon, stride));
   s->H_done = horizon; s->stride = stride;

@@ -61,13 +61,13 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, rs));
     KParams Pf = s->P;
     Pf.state = s->replay; Pf.tape = tapes[buf]; Pf.tape_flag = tflags[buf];
-    if (s->chunk > 0) {   // envs in the order of the work the segment after this one took (the tape written last, on this stream or before ev_fwd)
+    if (s->sort_mode) {   // envs in the order of the work the segment after this one took (the tape written last, on this stream or before ev_fwd)
       const int src = overlap ? ((g + 1) & 1) : 0;
-      if (g + 1 < nseg && s->stat_rep_valid[src]) { CU(sort_envs(s, s->stat_rep[src], 0, 4, s->perm_rep, rs)); Pf.perm = s->perm_rep; }
+      if ((s->sort_mode & 2) && g + 1 < nseg && s->stat_rep_valid[src]) { CU(sort_envs(s, s->stat_rep[src], 0, 4, s->perm_rep, rs)); Pf.perm = s->perm_rep; }
       Pf.stat = s->stat_rep[buf];
     }
     CU(launch_forward(s, Pf, t0, t1, 0, true, rs));
-    s->stat_rep_valid[buf] = s->chunk > 0;
+    s->stat_rep_valid[buf] = s->sort_mode != 0;
     if (overlap) CU(cudaEventRecord(s->ev_rep[buf], rs));
     return DLO_OK;
   };
@@ -91,7 +91,7 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
     Pa.tape = tapes[buf]; Pa.tape_flag = tflags[buf]; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
-    if (s->chunk > 0 && s->stat_rep_valid[buf]) {   // envs whose substeps must be recomputed (self-contact corrections) share CTAs
+    if ((s->sort_mode & 4) && s->stat_rep_valid[buf]) {   // envs whose substeps must be recomputed (self-contact corrections) share CTAs
       CU(sort_envs(s, s->stat_rep[buf], 1, 0, s->perm_main, s->stream));
       Pa.perm = s->perm_main;
     }
