@@ -234,6 +234,8 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
   EnvConst<VPL> c;
   load_env<VPL>(P, env, tp, c);
   warp_setup<VPL>(P, env, tp.lane, sm);
+  // work: self-contact work units of this launch; npen: which tenths of the launch's substeps applied a self-contact
+  // correction (bit 9 = the last tenth) - envs with the same pattern recompute the same substeps in the adjoint
   int work = 0, npen = 0;
   const size_t blk = (size_t)STATE_ROWS * P.NS, rec = (size_t)tape_rows(P.N_C) * P.NS;
   LaneState<VPL> s;
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
       } else {
         substep<VPL, 0>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
       }
-      work += R.work; npen += R.any_pen;
+      work += R.work; npen |= R.any_pen << ((((t - t0) * P.n_sub + sub) * 10) / ((t1 - t0) * P.n_sub));
     }
     if (stride > 0 && (t + 1) % stride == 0) store_state<VPL>(P.ckpt + ((size_t)((t + 1) / stride) * P.B + env) * blk, tp.base, P.NS, s);
   }

@@ -48,7 +48,7 @@ struct KParams {
   float* gmat;           // [B][5] running material gradient
   float* g_actions;      // [H][B][G][6] (may be null)
   const int* perm;       // [B] env handled by warp slot i (null: identity); set per launch, sorted by the envs' recent self-contact work
-  int* stat;             // [B][2] written at the end of a forward launch: self-contact work units, substeps with a correction
+  int* stat;             // [B][2] written at the end of a forward launch: self-contact work units, time pattern of the substeps with a correction
   uint8_t* tape_flag;    // [stride*n_sub][B]: 1 if the substep applied a self-contact correction (written by the replay)
   // per-warp shared memory layout (float offsets from the warp's base), set by the host
   int sm_pose, sm_prim, sm_q, sm_ys, sm_acc, sm_vs, sm_mid, sm_dp, sm_cand, sm_lam, sm_dpbar, sm_ybar, sm_vbar, sm_posebar, sm_blk, sm_xref, sm_hot, sm_warp_floats;
