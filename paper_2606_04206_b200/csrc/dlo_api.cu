@@ -37,6 +37,9 @@ struct dlo_sim {
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
   float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
   uint8_t *kin = nullptr, *pins = nullptr, *tape_flag = nullptr, *tape_flag2 = nullptr;
+  float* side[2] = {nullptr, nullptr};   // side-record pools, slot counters and slot indices of the two tape buffers
+  int *side_count[2] = {nullptr, nullptr}, *tape_slot[2] = {nullptr, nullptr};
+  int side_cap = 0, side_floats = 0;
   float* tape2 = nullptr;            // second tape buffer: the replay of segment g-1 overlaps the adjoint of segment g
   cudaStream_t aux = nullptr;
   cudaEvent_t ev_fwd = nullptr, ev_rep[2] = {nullptr, nullptr}, ev_adj[2] = {nullptr, nullptr};
@@ -241,7 +244,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
+                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->side[0], s->side[1], s->side_count[0], s->side_count[1], s->tape_slot[0], s->tape_slot[1], s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
   for (void* p : dev) if (p) cudaFree(p);
   if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
   for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
@@ -385,6 +388,28 @@ static dlo_status ensure_tape(dlo_sim* s, int H, int stride) {
     CU(dalloc(&s->tape, seg * B * rec));
     CU(dalloc(&s->tape_flag, seg * B));
     s->tape_blocks = seg;
+    for (int k = 0; k < 2; ++k) {
+      for (void* p : {(void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
+      s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
+    }
+    s->side_cap = 0;
+  }
+  if (s->P.self_contact && !getenv("DLO_NO_SIDE")) {
+    // side records for one substep in twelve (config 5 uses one in thirty); a substep that finds the pool empty is
+    // recomputed by the reverse pass instead.  Optional: without the memory the reverse pass recomputes them all.
+    s->side_floats = side_record_floats(s->P, 33 * s->VPL);
+    s->side_cap = (int)std::min<size_t>((size_t)1 << 30, std::max<size_t>(1024, s->tape_blocks * B / 12));
+    for (int k = 0; k < (nseg > 1 ? 2 : 1); ++k) {
+      if (s->side[k]) continue;
+      const bool ok = cudaMalloc((void**)&s->side[k], (size_t)s->side_cap * s->side_floats * sizeof(float)) == cudaSuccess &&
+                      cudaMalloc((void**)&s->side_count[k], sizeof(int)) == cudaSuccess &&
+                      cudaMalloc((void**)&s->tape_slot[k], s->tape_blocks * B * sizeof(int)) == cudaSuccess;
+      if (!ok) {
+        cudaGetLastError();
+        for (void* p : {(void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
+        s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
+      }
+    }
   }
   if (nseg > 1 && !s->tape2) {
     if (cudaMalloc((void**)&s->tape2, s->tape_blocks * B * rec * sizeof(float)) != cudaSuccess ||
@@ -432,6 +457,10 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     const int buf = (two && ((nseg - 1) & 1)) ? 1 : 0;
     Pf.tape = buf ? s->tape2 : s->tape;
     Pf.tape_flag = buf ? s->tape_flag2 : s->tape_flag;
+    if (s->side[buf]) {
+      CU(cudaMemsetAsync(s->side_count[buf], 0, sizeof(int), s->stream));
+      Pf.side = s->side[buf]; Pf.side_count = s->side_count[buf]; Pf.tape_slot = s->tape_slot[buf]; Pf.side_cap = s->side_cap; Pf.side_floats = s->side_floats;
+    }
     if (s->sort_mode) {
       Pf.stat = s->stat_rep[buf];
       if ((s->sort_mode & 1) && s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }

@@ -61,6 +61,10 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, rs));
     KParams Pf = s->P;
     Pf.state = s->replay; Pf.tape = tapes[buf]; Pf.tape_flag = tflags[buf];
+    if (s->side[buf]) {
+      CU(cudaMemsetAsync(s->side_count[buf], 0, sizeof(int), rs));
+      Pf.side = s->side[buf]; Pf.side_count = s->side_count[buf]; Pf.tape_slot = s->tape_slot[buf]; Pf.side_cap = s->side_cap; Pf.side_floats = s->side_floats;
+    }
     if (s->sort_mode) {   // envs in the order of the work the segment after this one took (the tape written last, on this stream or before ev_fwd)
       const int src = overlap ? ((g + 1) & 1) : 0;
       if ((s->sort_mode & 2) && g + 1 < nseg && s->stat_rep_valid[src]) { CU(sort_envs(s, s->stat_rep[src], 0, 4, s->perm_rep, rs)); Pf.perm = s->perm_rep; }
@@ -91,6 +95,7 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
     Pa.tape = tapes[buf]; Pa.tape_flag = tflags[buf]; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
+    if (s->side[buf]) { Pa.side = s->side[buf]; Pa.tape_slot = s->tape_slot[buf]; Pa.side_floats = s->side_floats; Pa.side_cap = s->side_cap; }
     if ((s->sort_mode & 4) && s->stat_rep_valid[buf]) {   // envs whose substeps must be recomputed (self-contact corrections) share CTAs
       CU(sort_envs(s, s->stat_rep[buf], 1, 0, s->perm_main, s->stream));
       Pa.perm = s->perm_main;

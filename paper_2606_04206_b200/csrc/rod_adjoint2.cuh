@@ -53,7 +53,7 @@ __device__ __forceinline__ void edge_reverse_pre(const f3& epred, float lam, flo
 template <int VPL>
 __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL>& tp, const EnvConst<VPL>& c, const WarpSmem& sm, int env,
                                                 const float ap[6], const float ac[6], int sub, const float* __restrict__ s0blk,
-                                                const float* __restrict__ s1blk, LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag) {
+                                                const float* __restrict__ s1blk, LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag, int side_slot) {
   const float h = P.h, inv_h = P.inv_h;
   // ---- forward recompute with recording.  The start state is read from the tape twice (here and again for the
   // reverse of A2) rather than held in ~70 registers across the projection loop, the hottest part of the kernel.
@@ -68,8 +68,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   if (P.G > 0) {
     for (int k = tp.lane; k < P.G * 24; k += 32) sm.posebar[k] = 0.0f;
   }
-  if (contact_flag) {
-    // the substep applied a self-contact correction: recompute it with recording (candidate list, depth sums, corrections)
+  if (contact_flag == 1) {
+    // the substep applied a self-contact correction and left no side record: recompute it with recording (candidate list, depth sums, corrections)
     ContactCache<VPL> cc;
     cc.reset(-1.0f);
     substep<VPL, 1>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc, const_cast<float*>(s0blk) + (size_t)TAPE_LAM * P.NS);
@@ -88,6 +88,23 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       R.t_old[k] = ec0.t[k];
     }
     R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
+    if (contact_flag == 2) {
+      // self-contact data of the substep from its side record: candidate list, depth sums, v^1 (v^3 includes friction here);
+      // the summed corrections of the Jacobi passes are read from the record in the reverse loop
+      const float* sr = P.side + (size_t)side_slot * P.side_floats;
+      R.ncand = reinterpret_cast<const int*>(sr)[0];
+      R.jac_mask = reinterpret_cast<const unsigned*>(sr)[1];
+      R.any_pen = 1;
+      load_rows3<VPL>(sr + side_off_v1(), tp.base, P.NS, R.v1);
+      const unsigned* cs = reinterpret_cast<const unsigned*>(sr + side_off_cand(P));
+      unsigned* cd = reinterpret_cast<unsigned*>(sm.cand);
+      for (int p = tp.lane; p < (R.ncand + 1) / 2; p += 32) cd[p] = cs[p];
+      for (int p = tp.lane; p < R.ncand; p += 32) sm.dp[p] = sr[side_off_dp(P) + p];
+#pragma unroll
+      for (int k = 0; k < VPL; ++k) sm.mid[4 * sm.NP + vpos<VPL>(tp.base + k)] = c.w[k];
+      acc_tape = const_cast<float*>(sr) + side_off_acc(P);
+      __syncwarp();
+    }
     // state at the end of the substep = start state of the next record (positions and directors are all that is used)
     load_rows3<VPL>(s1blk + (size_t)ROW_X * P.NS, tp.base, P.NS, s.x);
     load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
@@ -429,8 +446,9 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
       const size_t rec = (size_t)tape_rows(P.N_C) * P.NS, idx = (size_t)(t - t0) * P.n_sub + sub;
       const float* s0blk = P.tape + (idx * P.B + env) * rec;
       const float* s1blk = P.tape + ((idx + 1) * P.B + env) * rec;
-      const int cflag = P.tape_flag ? (int)P.tape_flag[(size_t)((t - t0) * P.n_sub + sub) * P.B + env] : 1;
-      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, s1blk, A, G, acc_tape, cflag);
+      const int cflag = P.tape_flag ? (int)P.tape_flag[idx * P.B + env] : 1;
+      const int slot = (cflag == 2) ? P.tape_slot[idx * P.B + env] : -1;
+      substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, s1blk, A, G, acc_tape, cflag, slot);
     }
     if (P.g_actions && tp.lane < P.G) {
       float* gc = P.g_actions + (((size_t)t * P.B + env) * P.G + tp.lane) * 6;

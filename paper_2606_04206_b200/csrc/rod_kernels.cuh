@@ -263,7 +263,18 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
 #pragma unroll
         for (int k = 0; k < VPL; ++k) am[k] = __uint_as_float(R.active[k]);
         store_row<VPL>(tb + (size_t)TAPE_ACT * P.NS, tp.base, P.NS, am);
-        if (tp.lane == 0) P.tape_flag[idx * P.B + env] = (uint8_t)R.any_pen;
+        int flag = R.any_pen;
+        if (R.any_pen && R.side_slot >= 0) {   // what the reverse pass needs of this substep's self-contact, so that it need not recompute it
+          float* sr = P.side + (size_t)R.side_slot * P.side_floats;
+          if (tp.lane == 0) { reinterpret_cast<int*>(sr)[0] = R.ncand; reinterpret_cast<unsigned*>(sr)[1] = R.jac_mask; P.tape_slot[idx * P.B + env] = R.side_slot; }
+          store_rows3<VPL>(sr + side_off_v1(), tp.base, P.NS, R.v1);
+          const unsigned* cs = reinterpret_cast<const unsigned*>(sm.cand);
+          unsigned* cd = reinterpret_cast<unsigned*>(sr + side_off_cand(P));
+          for (int p = tp.lane; p < (R.ncand + 1) / 2; p += 32) cd[p] = cs[p];
+          for (int p = tp.lane; p < R.ncand; p += 32) sr[side_off_dp(P) + p] = sm.dp[p];
+          flag = 2;
+        }
+        if (tp.lane == 0) P.tape_flag[idx * P.B + env] = (uint8_t)flag;
       } else {
         substep<VPL, 0>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc);
       }

@@ -62,6 +62,7 @@ template <int VPL> struct SubRec {
   float S[VPL];
   unsigned active[VPL];   // bit k<K: primitive k responded; bit K+2g+f: finger f of gripper g responded
   int ncand, any_pen;
+  int side_slot;          // MODE 2: slot of this substep's side record (-1: none)
   int work;               // rough count of the self-contact work this substep did (scheduling hint only)
   unsigned jac_mask;      // bit it: the Jacobi pass of iteration it applied at least one correction
 };
@@ -519,7 +520,8 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // leaves r_sum / 2 of slack: a full filter every few tens of substeps.  The near ones are measured again at every
   // x^p (filter_near) and swept when they can penetrate within the iteration's max |dx|.  A pass that cannot apply a
   // correction changes nothing, so the state is identical to building the whole list and sweeping it every time.
-  R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u; R.work = 0;
+  R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u; R.work = 0; R.side_slot = -1;
+  bool side_tried = false;
   bool built = false;
   float D1 = 0.0f;
   float dnear = 1.0e30f;   // exact minimum distance at x^p over the pairs of the candidate list in use
@@ -738,6 +740,13 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       R.work += any ? 3 : 1;
       __syncwarp();
       if (any) {
+        if (MODE == 2 && P.side && !side_tried) {   // replay: the corrections go to a side record (if the pool has a slot left)
+          side_tried = true;
+          int sl = 0;
+          if (tp.lane == 0) sl = atomicAdd(P.side_count, 1);
+          sl = __shfl_sync(DLO_FULL, sl, 0);
+          if (sl < P.side_cap) { R.side_slot = sl; acc_tape = P.side + (size_t)sl * P.side_floats + side_off_acc(P); }
+        }
         R.any_pen = 1;
         R.jac_mask |= 1u << it;
 #pragma unroll
@@ -745,7 +754,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
           const int i = vpos<VPL>(tp.base + k);   // own vertex, slot-major position
           const f3 a = lds3(sm.acc, sm.NP, i);
           R.dx[k] += a;
-          if (REC) sts3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i, a);
+          if (MODE >= 1 && acc_tape) sts3(acc_tape + (size_t)it * 3 * sm.NP, sm.NP, i, a);
           sts3(sm.acc, sm.NP, i, zero3<float>());
         }
         __syncwarp();

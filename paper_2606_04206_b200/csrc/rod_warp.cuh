@@ -47,6 +47,12 @@ struct KParams {
   float* acc_tape;       // [B][N_C][3][32*VPL] self-contact corrections of the substep being reversed
   float* gmat;           // [B][5] running material gradient
   float* g_actions;      // [H][B][G][6] (may be null)
+  // side records of the substeps that applied a self-contact correction (written by the replay, read by the adjoint
+  // instead of recomputing the substep): pool of side_cap slots of side_floats floats, slot index per tape record
+  float* side;
+  int* side_count;
+  int* tape_slot;        // [stride*n_sub][B]
+  int side_cap, side_floats;
   const int* perm;       // [B] env handled by warp slot i (null: identity); set per launch, sorted by the envs' recent self-contact work
   int* stat;             // [B][2] written at the end of a forward launch: self-contact work units, time pattern of the substeps with a correction
   uint8_t* tape_flag;    // [stride*n_sub][B]: 1 if the substep applied a self-contact correction (written by the replay)
@@ -74,6 +80,14 @@ __device__ __forceinline__ float warp_max(float v) { return __uint_as_float(__re
 __device__ __forceinline__ float warp_min(float v) { return __uint_as_float(__reduce_min_sync(DLO_FULL, __float_as_uint(v))); }
 __device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
 __device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
+
+// layout of a side record (float offsets): header (ncand, jac_mask), v^1 rows, candidate codes, depth sums D_p, the summed
+// corrections of every Jacobi pass [N_C][3][33 VPL]
+__host__ __device__ inline int side_off_v1() { return 4; }
+__host__ __device__ inline int side_off_cand(const KParams& P) { return 4 + 3 * P.NS; }
+__host__ __device__ inline int side_off_dp(const KParams& P) { return side_off_cand(P) + P.cand_cap / 2; }
+__host__ __device__ inline int side_off_acc(const KParams& P) { return side_off_dp(P) + P.cand_cap; }
+__host__ __device__ inline int side_record_floats(const KParams& P, int NP) { return (side_off_acc(P) + P.N_C * 3 * NP + 3) / 4 * 4; }
 
 template <int VPL> struct Topo {
   int lane, base, nv, ks, nl, pl;   // own lane, first vertex, #valid vertices, last valid slot, next / previous lane
