@@ -122,6 +122,27 @@ def test_gradient_independent_of_stride(dlo):
             assert np.abs(o[k] - outs[0][k]).max() <= 5e-5 * np.abs(outs[0][k]).max(), k
 
 
+@pytest.mark.parametrize("cfg, H, stride, tol", [(4, 400, 40, 5e-5), (5, 300, 100, 1e-3)])
+def test_side_records_equal_recompute(dlo, monkeypatch, cfg, H, stride, tol):
+    """A substep that applied a self-contact correction is reversed either from the side record the replay left, or,
+    when the pool has no slot (here: DLO_NO_SIDE, no pool at all), by recomputing it inside the adjoint kernel.  Same
+    trajectory, same arithmetic per substep: the gradients agree to rounding level (shared-memory atomics aside)."""
+    P = make_problem(cfg, batch=16, horizon=H)
+    outs = []
+    for no_side in (False, True):
+        monkeypatch.delenv("DLO_NO_SIDE", raising=False)
+        if no_side:
+            monkeypatch.setenv("DLO_NO_SIDE", "1")
+        sim = dlo.DloSim(P)
+        x = sim.rollout(H, stride).state()["x"]
+        _, seed = loss_and_seed(P, x)
+        outs.append(sim.backward(seed))
+        sim.close()
+    assert np.abs(outs[0]["g_x0"]).max() > 0
+    for k in ("g_actions", "g_x0", "g_v0", "g_material"):
+        assert np.abs(outs[1][k] - outs[0][k]).max() <= tol * np.abs(outs[0][k]).max(), k
+
+
 # Kinked cases (DESIGN.md "gradients at branch thresholds"): Eq.11 drives every active hinge onto its yield surface
 # and resting contact sits on the f = 1 / approach thresholds, where the step is continuous but its derivative jumps.
 # There the oracle's own gradient moves by far more than 1e-3 when its inputs move by one fp32 rounding, so no fp32
