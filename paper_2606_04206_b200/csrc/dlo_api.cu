@@ -143,7 +143,12 @@ size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
     const size_t tape = ((size_t)(stride < horizon ? stride : horizon) * P.n_sub + 1) * B * tape_rows(P.N_C) * P.NS * sizeof(float);
     n += tape * (horizon > stride ? 2 : 1);                                     // tape of one segment, double-buffered when there are several
     n += B * blk;                                                              // running adjoint
-    if (P.self_contact) n += B * (size_t)P.N_C * 3 * 33 * vpl_for(P.N) * 4;    // self-contact correction tape
+    if (P.self_contact) {
+      n += B * (size_t)P.N_C * 3 * 33 * vpl_for(P.N) * 4;    // self-contact correction tape
+      const size_t seg = (size_t)(stride < horizon ? stride : horizon) * P.n_sub + 1, cap = std::max<size_t>(1024, seg * B / 12);
+      n += (horizon > stride ? 2 : 1) * (cap * side_record_floats(P, 33 * vpl_for(P.N)) * 4 + seg * B * 4 + 4);   // side-record pools + slot indices
+    }
+    n += 3 * B * 8 + 2 * B * 4;                                                // work statistics and env orders
   }
   return n;
 }
