@@ -56,14 +56,24 @@ __device__ __forceinline__ void posebar_add(float* dst, const PoseBar<float>& g)
 #pragma unroll
   for (int k = 0; k < 9; ++k) atomicAdd(dst + 3 + k, g.R[k]);
 }
-__device__ __forceinline__ void grasp_target_adj(const KParams& P, const WarpSmem& sm, int code, const f3& tbar) {
-  const int slot = code - KIN_GRASP0, g = slot / P.M;
-  const float* q = sm.q + 3 * slot;
+// Adjoint of the grasp targets p1 + R1 q of a lane's kinematic vertices, summed per gripper in registers and added to
+// the shared pose adjoint once (flush): consecutive vertices of a lane usually hang on the same gripper, and a
+// shared-memory float atomicAdd is a compare-and-swap loop (twelve of them per vertex otherwise).
+struct GraspAcc {
   PoseBar<float> b;
-  pose_bar_zero(b);
-  rigid_point_adj<float>(mk3<float>(q[0], q[1], q[2]), tbar, b);
-  posebar_add(sm.posebar + g * 24 + 12, b);
-}
+  int g;
+  __device__ __forceinline__ void init() { pose_bar_zero(b); g = -1; }
+  __device__ __forceinline__ void flush(const WarpSmem& sm) {
+    if (g >= 0) posebar_add(sm.posebar + g * 24 + 12, b);
+    g = -1;
+  }
+  __device__ __forceinline__ void add(const KParams& P, const WarpSmem& sm, int code, const f3& tbar) {
+    const int slot = code - KIN_GRASP0, gg = slot / P.M;
+    if (gg != g) { flush(sm); pose_bar_zero(b); g = gg; }
+    const float* q = sm.q + 3 * slot;
+    rigid_point_adj<float>(mk3<float>(q[0], q[1], q[2]), tbar, b);
+  }
+};
 
 // one rigid body (primitive b < K, else finger (b-K)) evaluated at y: phi, n, body velocity
 __device__ __forceinline__ bool body_eval(const KParams& P, const WarpSmem& sm, int b, const f3& y, float& phi, f3& n, f3& vb) {

@@ -163,13 +163,16 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   phase_sync(sm);
   // ---- reverse A8 commit
   f3 velbar[VPL];
+  GraspAcc ga;
+  ga.init();
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
     velbar[k] = zero3<float>();
     if (c.kin[k] == KIN_FREE) velbar[k] = axpy(A.v[k], h, A.x[k]);
-    else if (c.kin[k] >= KIN_GRASP0) { grasp_target_adj(P, sm, c.kin[k], A.x[k]); velbar[k] = A.v[k]; A.x[k] = zero3<float>(); }
+    else if (c.kin[k] >= KIN_GRASP0) { ga.add(P, sm, c.kin[k], A.x[k]); velbar[k] = A.v[k]; A.x[k] = zero3<float>(); }
     A.v[k] = zero3<float>();
   }
+  ga.flush(sm);
 
   {   // old tangents (frame transport) -> old positions, while the old edge geometry is still at hand
     f3 send = zero3<float>();
@@ -337,10 +340,11 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
       G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], R.v1[k]);
     } else if (c.kin[k] >= KIN_GRASP0) {
       const f3 tb = inv_h * v1bar[k];
-      grasp_target_adj(P, sm, c.kin[k], tb);
+      ga.add(P, sm, c.kin[k], tb);
       A.x[k] -= tb;
     }
   }
+  ga.flush(sm);
 
   phase_sync(sm);
   // ---- reverse A2 forces: bending elements (and the stretch force in ENERGY mode) -> old edge geometry
