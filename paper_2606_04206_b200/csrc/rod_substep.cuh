@@ -505,12 +505,17 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     R.xp[k] = axpy(s.x[k], h, v1);
     R.dx[k] = zero3<float>();
     R.S[k] = 0.0f;
-    R.t_old[k] = ec.t[k];
   }
   const f3 xpr = shfl3(R.xp[0], tp.nl);
   f3 epred[VPL];   // predicted edge vectors, constant during the projection loop
 #pragma unroll
   for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
+  // x^p is x + h v^1: recomputed where it is read (one FFMA per component) instead of held in 3 VPL registers across the
+  // projection loop.  `h2` is h made opaque, or the compiler would merge the recomputation with R.xp (kept for the tape
+  // in MODE 1, 2) and keep it in registers; same operands, same rounding, same bits.
+  float h2 = h;
+  asm volatile("" : "+f"(h2));
+  auto XP = [&](int k) { return axpy(s.x[k], h2, R.v1[k]); };
 
   // Self-contact is evaluated lazily (exactly): segment distance is 1-Lipschitz in the end points, so with d_ref the
   // minimum distance of a set of pairs at the positions x_ref where they were last measured, none of them can
@@ -529,7 +534,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     float m2 = 0.0f;
 #pragma unroll
     for (int k = 0; k < VPL; ++k)
-      if (tp.vvalid[k]) { const f3 d = R.xp[k] - cc.xref[k]; m2 = fmaxf(m2, dot(d, d)); }
+      if (tp.vvalid[k]) { const f3 d = XP(k) - cc.xref[k]; m2 = fmaxf(m2, dot(d, d)); }
     D1 = sqrt_(warp_max(m2));
   }
   auto build_list = [&](bool vote) {
@@ -542,7 +547,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       float m2 = 0.0f;
 #pragma unroll
       for (int k = 0; k < VPL; ++k)
-        if (tp.vvalid[k]) { const f3 d = R.xp[k] - lds3(sm.xref, sm.NP, vpos<VPL>(tp.base + k)); m2 = fmaxf(m2, dot(d, d)); }
+        if (tp.vvalid[k]) { const f3 d = XP(k) - lds3(sm.xref, sm.NP, vpos<VPL>(tp.base + k)); m2 = fmaxf(m2, dot(d, d)); }
       const float lm = 0.999f * P.list_margin;
       const float wm = warp_max(m2);
       fresh = !(wm <= lm * lm);
@@ -552,15 +557,15 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
       const int i = vpos<VPL>(tp.base + k);
-      sts3(sm.ys, sm.NP, i, R.xp[k]);
+      sts3(sm.ys, sm.NP, i, XP(k));
       sm.mid[4 * sm.NP + i] = c.w[k];
     }
     if (fresh) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {
         const int i = vpos<VPL>(tp.base + k);
-        sts3(sm.xref, sm.NP, i, R.xp[k]);
-        sts3(sm.mid, sm.NP, i, axpy(R.xp[k], 0.5f, epred[k]));
+        sts3(sm.xref, sm.NP, i, XP(k));
+        sts3(sm.mid, sm.NP, i, axpy(XP(k), 0.5f, epred[k]));
         sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
       }
       // bounding sphere of this lane's edge block (centre = mean of its edge midpoints)
@@ -568,13 +573,13 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       float bn = 0.0f, brad = -1.0e30f;
 #pragma unroll
       for (int k = 0; k < VPL; ++k)
-        if (tp.evalid[k]) { bc += axpy(R.xp[k], 0.5f, epred[k]); bn += 1.0f; }
+        if (tp.evalid[k]) { bc += axpy(XP(k), 0.5f, epred[k]); bn += 1.0f; }
       if (bn > 0.0f) {
         bc = (1.0f / bn) * bc;
 #pragma unroll
         for (int k = 0; k < VPL; ++k)
           if (tp.evalid[k]) {
-            const f3 dm = axpy(R.xp[k], 0.5f, epred[k]) - bc;
+            const f3 dm = axpy(XP(k), 0.5f, epred[k]) - bc;
             brad = fmaxf(brad, sqrt_(dot(dm, dm)) + 0.5f * sqrt_(dot(epred[k], epred[k])));
           }
       }
@@ -608,7 +613,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     cc.nhot = co.nhot;
     dnear = co.dmin;
 #pragma unroll
-    for (int k = 0; k < VPL; ++k) cc.xref[k] = R.xp[k];
+    for (int k = 0; k < VPL; ++k) cc.xref[k] = XP(k);
     for (int p = tp.lane; p < R.ncand; p += 32) {
       float d = 0.0f;
       const unsigned code = sm.cand[p];
@@ -631,7 +636,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     } else if (P.self_contact && cc.nhot > 0) {
       // the far pairs are safe where they are: measure the near ones at x^p, they are this substep's candidates
 #pragma unroll
-      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k]);
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), XP(k));
       __syncwarp();
       const CandOut co = filter_near<VPL>(P, tp.lane, sm.base, cc.nhot);
       R.work += 1;
@@ -734,7 +739,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     }
     if (sweep && R.ncand > 0) {
 #pragma unroll
-      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]);
+      for (int k = 0; k < VPL; ++k) sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), XP(k) + R.dx[k]);
       __syncwarp();
       const bool any = contact_pass<VPL>(P, tp.lane, sm.base, R.ncand);
       R.work += any ? 3 : 1;
@@ -768,7 +773,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) vel[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k];
   if (P.self_contact && R.any_pen) {
 #pragma unroll
-    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), R.xp[k] + R.dx[k]); sts3(sm.vs, sm.NP, vpos<VPL>(tp.base + k), vel[k]); }
+    for (int k = 0; k < VPL; ++k) { sts3(sm.ys, sm.NP, vpos<VPL>(tp.base + k), XP(k) + R.dx[k]); sts3(sm.vs, sm.NP, vpos<VPL>(tp.base + k), vel[k]); }
     __syncwarp();
     friction_pass<VPL>(P, tp.lane, sm.base, R.ncand, c.mu_s);
     __syncwarp();
@@ -788,12 +793,23 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     R.v3[k] = vel[k];
     R.active[k] = 0u;
     if (c.kin[k] == KIN_FREE && (P.K > 0 || P.G > 0)) {
-      const CoupleOut co = rigid_coupling(P, sm.prim, sm.pose, R.xp[k] + R.dx[k], vel[k], c.mu_r);
+      const CoupleOut co = rigid_coupling(P, sm.prim, sm.pose, XP(k) + R.dx[k], vel[k], c.mu_r);
       vel[k] = co.v; R.active[k] = co.active;
     }
     R.v4[k] = vel[k];
   }
 
+  // tangents of the positions the substep started from, for the frame transport of A9: recomputed here (the expression of
+  // edge_refresh, same bits as ec.t had) rather than held in 3 VPL registers across the projection loop
+  {
+    const f3 xr = shfl3(s.x[0], tp.nl);
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      const f3 e = next_of<VPL>(s.x, xr, k, tp.ks) - s.x[k];
+      const float iL = tp.evalid[k] ? rsqrt_(dot(e, e)) : 0.0f;
+      R.t_old[k] = iL * e;
+    }
+  }
   // -- A8 commit
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
