@@ -191,32 +191,6 @@ template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<
 // Persistent forward segment: steps t0..t1-1 of every env, one warp per env, state in registers throughout.
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  write_tape: the state at
 // the start of every substep goes to P.tape (replay half of the reverse pass).
-// rows of one tape record (per substep and env), each NS floats: the state at the start of the substep, then what the
-// reverse pass would otherwise have to recompute: predicted positions, final corrections, the velocity before the rigid
-// coupling (differencing positions would cost too many digits), Eq.10 multiplier sums, the
-// mask of rigid bodies that responded, and the multipliers of every iteration
-enum { TAPE_XP = STATE_ROWS, TAPE_DX = TAPE_XP + 3, TAPE_V3 = TAPE_DX + 3, TAPE_S = TAPE_V3 + 3, TAPE_ACT = TAPE_S + 1, TAPE_LAM = TAPE_ACT + 1 };
-__host__ __device__ inline int tape_rows(int N_C) { return TAPE_LAM + N_C; }
-
-template <int VPL> __device__ __forceinline__ void store_rows3(float* __restrict__ rows, int base, int NS, const f3 a[VPL]) {
-  float r[VPL];
-#pragma unroll
-  for (int k = 0; k < VPL; ++k) r[k] = a[k].x;
-  store_row<VPL>(rows, base, NS, r);
-#pragma unroll
-  for (int k = 0; k < VPL; ++k) r[k] = a[k].y;
-  store_row<VPL>(rows + NS, base, NS, r);
-#pragma unroll
-  for (int k = 0; k < VPL; ++k) r[k] = a[k].z;
-  store_row<VPL>(rows + 2 * NS, base, NS, r);
-}
-template <int VPL> __device__ __forceinline__ void load_rows3(const float* __restrict__ rows, int base, int NS, f3 a[VPL]) {
-  float rx[VPL], ry[VPL], rz[VPL];
-  load_row<VPL>(rows, base, NS, rx); load_row<VPL>(rows + NS, base, NS, ry); load_row<VPL>(rows + 2 * NS, base, NS, rz);
-#pragma unroll
-  for (int k = 0; k < VPL; ++k) a[k] = mk3<float>(rx[k], ry[k], rz[k]);
-}
-
 // Persistent forward segment: steps t0..t1-1 of every env, one warp per env, state in registers throughout.
 // stride > 0: checkpoint (t+1)/stride written after every `stride`-th step (L115).  TAPE = true is the replay half of
 // the reverse pass: a tape record per substep goes to P.tape, and the segment's final state to record [n_substeps].
@@ -255,7 +229,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
         float* tb = P.tape + (idx * P.B + env) * rec;
         store_state<VPL>(tb, tp.base, P.NS, s);
         substep<VPL, 2>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc, tb + (size_t)TAPE_LAM * P.NS);
-        store_rows3<VPL>(tb + (size_t)TAPE_XP * P.NS, tp.base, P.NS, R.xp);
+        // (the x^p rows are stored inside substep, as soon as they exist: fewer registers live across its projection loop)
         store_rows3<VPL>(tb + (size_t)TAPE_DX * P.NS, tp.base, P.NS, R.dx);
         store_rows3<VPL>(tb + (size_t)TAPE_V3 * P.NS, tp.base, P.NS, R.v3);
         store_row<VPL>(tb + (size_t)TAPE_S * P.NS, tp.base, P.NS, R.S);

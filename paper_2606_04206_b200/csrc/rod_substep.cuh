@@ -510,6 +510,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   f3 epred[VPL];   // predicted edge vectors, constant during the projection loop
 #pragma unroll
   for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
+  if (MODE == 2 && lam_rows) store_rows3<VPL>(lam_rows + (ptrdiff_t)(TAPE_XP - TAPE_LAM) * P.NS, tp.base, P.NS, R.xp);   // replay: x^p rows of the tape record
   // x^p is x + h v^1: recomputed where it is read (one FFMA per component) instead of held in 3 VPL registers across the
   // projection loop.  `h2` is h made opaque, or the compiler would merge the recomputation with R.xp (kept for the tape
   // in MODE 1, 2) and keep it in registers; same operands, same rounding, same bits.

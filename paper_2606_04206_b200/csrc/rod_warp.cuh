@@ -140,6 +140,32 @@ template <int VPL> __device__ __forceinline__ void store_row(float* __restrict__
   }
 }
 
+// rows of one tape record (per substep and env), each NS floats: the state at the start of the substep, then what the
+// reverse pass would otherwise have to recompute: predicted positions, final corrections, the velocity before the rigid
+// coupling (differencing positions would cost too many digits), Eq.10 multiplier sums, the
+// mask of rigid bodies that responded, and the multipliers of every iteration
+enum { TAPE_XP = STATE_ROWS, TAPE_DX = TAPE_XP + 3, TAPE_V3 = TAPE_DX + 3, TAPE_S = TAPE_V3 + 3, TAPE_ACT = TAPE_S + 1, TAPE_LAM = TAPE_ACT + 1 };
+__host__ __device__ inline int tape_rows(int N_C) { return TAPE_LAM + N_C; }
+
+template <int VPL> __device__ __forceinline__ void store_rows3(float* __restrict__ rows, int base, int NS, const f3 a[VPL]) {
+  float r[VPL];
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].x;
+  store_row<VPL>(rows, base, NS, r);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].y;
+  store_row<VPL>(rows + NS, base, NS, r);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) r[k] = a[k].z;
+  store_row<VPL>(rows + 2 * NS, base, NS, r);
+}
+template <int VPL> __device__ __forceinline__ void load_rows3(const float* __restrict__ rows, int base, int NS, f3 a[VPL]) {
+  float rx[VPL], ry[VPL], rz[VPL];
+  load_row<VPL>(rows, base, NS, rx); load_row<VPL>(rows + NS, base, NS, ry); load_row<VPL>(rows + 2 * NS, base, NS, rz);
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) a[k] = mk3<float>(rx[k], ry[k], rz[k]);
+}
+
 // the per-lane slice of one env's state (x, v per vertex; d1 per edge; rest curvature per vertex)
 template <int VPL> struct LaneState {
   f3 x[VPL], v[VPL], d1[VPL];
