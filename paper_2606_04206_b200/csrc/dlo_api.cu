@@ -77,7 +77,7 @@ static int smem_layout(KParams& P, int VPL, bool adjoint) {
   if (P.self_contact) {
     P.sm_ys = take(3 * NP); P.sm_acc = take(3 * NP); P.sm_vs = take(3 * NP); P.sm_mid = take(5 * NP);
     P.sm_dp = take(P.cand_cap); P.sm_cand = take(P.cand_cap);   // candidates + prefilter survivors (ushort each)
-    P.sm_blk = take(4 * 32);
+    P.sm_blk = P.sm_vs;   // block bounding spheres (4 x 32 floats) live only inside build_pair_list; sm.vs is written after it (carry-over, friction)
     P.sm_hot = take(P.hot_cap / 2);   // near pairs (ushort each), kept across substeps
     if (!adjoint) P.sm_xref = take(3 * NP);   // positions at which the pair list was built (must outlive the substep)
   }
@@ -117,7 +117,9 @@ static void fill_params(const dlo_config& c, KParams& P) {
   P.n_sub = c.n_substeps; P.N_C = c.n_proj_iters; P.stretch_mode = c.stretch_mode; P.plasticity = c.enable_plasticity != 0;
   P.self_contact = c.enable_self_contact != 0; P.self_skip = c.self_skip;
   P.G = c.n_grippers; P.M = P.G ? c.n_grasp_max : 1; P.K = c.n_primitives;
-  P.cand_cap = round_up(4 * P.N, 32);
+  // 15/4 N pairs: with the block spheres aliased onto sm.vs this brings two 7-warp forward CTAs of config 5 under the
+  // 196 KB shared-memory configuration (97.5 KB each), which leaves the SM 60 KB of L1 for the spilled registers instead of 28
+  P.cand_cap = round_up(15 * P.N / 4, 32);
   P.hot_cap = 32 * vpl_for(P.N);   // <= a third of the 3 x 33 VPL floats of sm.vs, which holds two such arrays during a mid-loop rebuild
   P.list_margin = c.rope_radius;   // a quarter of the candidate distance 2(r_a+r_b)
   P.vote_mode = 3;

@@ -48,8 +48,8 @@ def test_scratch_bytes_matches_layout(dlo):
     blk = 11 * N * 4
     n = dlo.dlo_scratch_bytes(cfg, H, S)
     ckpt, tape = (H // S + 1) * B * blk, 2 * (S * 5 + 1) * B * (22 + 10) * N * 4     # two tape buffers of 22 + N_C rows per record
-    # two side-record pools (one substep in twelve; header, v^1, 512 candidate codes and depth sums, N_C x 3 x 132 corrections)
-    side = 2 * ((S * 5 + 1) * B // 12) * (4 + 3 * N + 256 + 512 + 10 * 3 * 132) * 4
+    # two side-record pools (one substep in twelve; header, v^1, 480 candidate codes and depth sums, N_C x 3 x 132 corrections)
+    side = 2 * ((S * 5 + 1) * B // 12) * (4 + 3 * N + 240 + 480 + 10 * 3 * 132) * 4
     assert n > ckpt + tape + side and n < ckpt + tape + side + 450e6
     assert dlo.dlo_scratch_bytes(cfg, H, 0) < 100e6          # forward only: constants + two state copies
     bad = make_config(dict(P["config"], n_verts=1000))
