@@ -33,9 +33,9 @@ UNIT = "env-steps/s"
 # substep 0.17 Mflop; forward+backward = forward + replay + reverse = 0.5 + 0.5 + 0.85 = 1.85 Mflop per env-step.
 FLOPS_PER_ENV_STEP = {"fwd": 0.5e6, "fwdbwd": 1.85e6}
 # DRAM bytes per env-substep of the dominant kernel (k_adjoint), from the `ncu --set full` capture summarised in
-# profiles/r01_final_ncu_summary.md: (34.831 GB read + 0.238 GB written) / (4096 envs x 100 frames x 5 substeps) = 17.1 KB,
+# profiles/r01_final_ncu_summary.md: (34.829 GB read + 0.237 GB written) / (4096 envs x 100 frames x 5 substeps) = 17.1 KB,
 # against 16.4 KB of tape record it has to read (algorithmic) plus the side records of the self-contact substeps.
-ADJ_DRAM_BYTES_PER_ENV_SUBSTEP = (34.831397e9 + 0.237687e9) / (4096 * 100 * 5)
+ADJ_DRAM_BYTES_PER_ENV_SUBSTEP = (34.829228e9 + 0.237290e9) / (4096 * 100 * 5)
 # fp32 ALU peak derived in DESIGN.md section 7: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
 ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
