@@ -23,7 +23,10 @@
  *   - Ownership: the caller owns every buffer it passes.  The library reads / writes them asynchronously on
  *     the stream given at create and keeps no pointer after the call returns, except `actions` (borrowed until
  *     the next dlo_set_actions / dlo_destroy: dlo_backward replays them).  Checkpoints, tape and per-env
- *     constants live in library-owned device memory (size: dlo_scratch_bytes).
+ *     constants live in library-owned device memory (size: dlo_scratch_bytes); so does the staging of the *_host
+ *     calls (per handle, freed by dlo_destroy).
+ *   - Device: a handle belongs to the CUDA device that was current at dlo_create; every later call on it must be
+ *     made with that device current (DLO_ERR_BAD_STATE otherwise).
  *   - Errors: every call returns a dlo_status; nothing aborts or throws across the ABI; a failed call leaves
  *     the handle usable.  dlo_last_error() returns a thread-local message for the last failing call.
  *   - Threading: one handle <-> one stream; calls are stream-ordered and (except the *_host calls and
@@ -104,6 +107,19 @@ dlo_status dlo_rollout_forward(dlo_sim* sim, int32_t horizon, int32_t checkpoint
 /* Current state; each pointer dev, may be NULL.  x, v, d1: [B][3][N]; kappa_bar: [B][2][N]. */
 dlo_status dlo_get_state(dlo_sim* sim, float* x, float* v, float* d1, float* kappa_bar);
 
+/* Exact restore (a checkpoint is "a single state"; the segment is re-run from it).  Puts back a
+ * state as dlo_get_state returned it, bit for bit: x, v, d1 dev [B][3][N], kappa_bar dev [B][2][N] (all four
+ * required), and `step_index`, the frame the next dlo_rollout_forward starts at: its step k uses the actions
+ * a_{step_index+k-1} -> a_{step_index+k} of the array given to dlo_set_actions (a_{-1} = init_pose), so
+ * step_index + horizon must not exceed that array.  No A0 runs: the frames are taken as given, and the grasp-local
+ * coordinates stay those captured by the last dlo_set_state (DLO_ERR_BAD_STATE if there was none, or if the scene
+ * changed since).  dlo_get_state -> dlo_restore_state -> rollout of k steps equals k more steps of the original
+ * rollout bitwise.  dlo_backward after such a rollout differentiates that segment only: g_actions [horizon][B][G][6]
+ * is indexed from step_index (the gradient with respect to a_{step_index-1} is dropped, like that of init_pose),
+ * g_x0 / g_v0 are with respect to the restored x, v.  dlo_set_state resets step_index to 0. */
+dlo_status dlo_restore_state(dlo_sim* sim, const float* x, const float* v, const float* d1, const float* kappa_bar,
+                             int32_t step_index);
+
 /* Reverse pass of the last checkpointed rollout.  Seeds dL/dx_T, dL/dv_T dev [B][3][N] (NULL = 0).  Outputs
  * (dev, each may be NULL, WRITTEN not accumulated): g_actions [H][B][G][6], g_x0, g_v0 [B][3][N],
  * g_material [B][5] = d/d(stretch, bend_stiffness, damping, yield_curv, creep_rate).  The initial frames and
@@ -111,6 +127,11 @@ dlo_status dlo_get_state(dlo_sim* sim, float* x, float* v, float* d1, float* kap
  * rollout. */
 dlo_status dlo_backward(dlo_sim* sim, const float* dL_dx_T, const float* dL_dv_T, float* g_actions, float* g_x0,
                         float* g_v0, float* g_material);
+
+/* After dlo_backward: the adjoint of the WHOLE start state of the rollout (what a chained segment-wise reverse pass
+ * hands to the segment before, L115).  Each pointer dev, may be NULL: g_x, g_v, g_d1 [B][3][N], g_kappa_bar [B][2][N].
+ * g_x, g_v equal dlo_backward's g_x0, g_v0.  DLO_ERR_BAD_STATE without a completed dlo_backward. */
+dlo_status dlo_get_state_adjoint(dlo_sim* sim, float* g_x, float* g_v, float* g_d1, float* g_kappa_bar);
 
 /* Host-buffer convenience calls (the end-to-end path): pageable or pinned HOST pointers, copies included, and
  * the call returns after the results have landed.  dlo_rollout_forward_host = set_state + set_actions +
@@ -126,7 +147,9 @@ dlo_status dlo_backward_host(dlo_sim* sim, const float* dL_dx_T, const float* dL
  * candidate list since dlo_set_state; n_bad (host, may be NULL) receives the number of such envs. */
 dlo_status dlo_check_numerics(dlo_sim* sim, int32_t* n_bad);
 
-/* Device bytes the library allocates for this config / rollout shape (constants + checkpoints + tape). */
+/* Device bytes the library allocates for this config / rollout shape (constants + checkpoints + tape).  A handle that
+ * is driven through the *_host calls additionally holds their device staging: 4 + 4 arrays [B][3][N], one [B][2][N],
+ * one [B][5] and two [H][B][G][6] (actions, action gradients). */
 size_t dlo_scratch_bytes(const dlo_config* cfg, int32_t horizon, int32_t checkpoint_stride);
 
 /* Number of kernel launches issued on this handle since create (bench.py's gpu_launches). */

@@ -37,6 +37,7 @@ struct oracle_sim {
   std::vector<EnvD> env;
   std::vector<double> actions;           // [H][B][G][6]
   int H_actions = 0, H_done = 0, stride = 0, record = 0;
+  int t_start = 0;                       // frame index of the state in s0 (0 after oracle_set_state; oracle_restore_state sets it)
 };
 
 static Config to_config(const oracle_config& o) {
@@ -152,6 +153,28 @@ void oracle_set_state(oracle_sim* h, const double* x0, const double* v0, const d
     (void)E;
   }
   h->H_done = 0;
+  h->t_start = 0;
+}
+
+// Harness plumbing (no arithmetic): put a full state (x, v, d1, kappa_bar as oracle_get_state returns them) back as the
+// start state of the next rollout, which then runs frames t_start, t_start+1, ... (a checkpoint is one
+// state; the segment is re-run from it).  No A0: the frames are taken as given; the grasp-local coordinates stay those
+// of the last oracle_set_state.  The reverse pass then differentiates that segment only (g_actions indexed from t_start).
+void oracle_restore_state(oracle_sim* h, const double* x, const double* v, const double* d1, const double* kbar, int32_t t_start) {
+  const Config& c = h->c; const int N = c.N, E = c.E();
+  for (int b = 0; b < h->B; ++b) {
+    EnvD& e = h->env[b];
+    State<double>& s = e.s0;
+    s.x.resize(N); s.v.resize(N); s.d1.resize(E); s.k1.assign(N, 0.0); s.k2.assign(N, 0.0);
+    const double* X = x + (size_t)b * 3 * N; const double* V = v + (size_t)b * 3 * N; const double* D = d1 + (size_t)b * 3 * N;
+    const double* Kb = kbar + (size_t)b * 2 * N;
+    for (int i = 0; i < N; ++i) { s.x[i] = mkv(X[i], X[N + i], X[2 * N + i]); s.v[i] = mkv(V[i], V[N + i], V[2 * N + i]); s.k1[i] = Kb[i]; s.k2[i] = Kb[N + i]; }
+    for (int j = 0; j < E; ++j) s.d1[j] = mkv(D[j], D[N + j], D[2 * N + j]);
+    e.cur = s;
+    e.ckpt.clear(); e.rec.clear();
+  }
+  h->H_done = 0;
+  h->t_start = t_start;
 }
 
 // Test hook: replace the A0 products (initial frames d1 [B][3][N], grasp-local coordinates q [B][G][M][3]) after
@@ -186,7 +209,8 @@ static const double* action_ptr(const oracle_sim* h, int b, int t) {   // a_t, t
 // record != 0: additionally keep the state after every step (for the pins that look at trajectories).
 int32_t oracle_rollout_forward(oracle_sim* h, int32_t horizon, int32_t stride, int32_t record) {
   const Config& c = h->c;
-  if (c.G > 0 && horizon > h->H_actions) return -1;
+  if (c.G > 0 && h->t_start + horizon > h->H_actions) return -1;
+  const int ts = h->t_start;
   h->stride = stride; h->record = record; h->H_done = horizon;
 #pragma omp parallel for schedule(dynamic)
   for (int b = 0; b < h->B; ++b) {
@@ -197,8 +221,8 @@ int32_t oracle_rollout_forward(oracle_sim* h, int32_t horizon, int32_t stride, i
     if (record) e.rec.push_back(e.cur);
     static const double none[1] = {0.0};
     for (int t = 0; t < horizon; ++t) {
-      const double* ap = c.G ? action_ptr(h, b, t - 1) : none;
-      const double* ac = c.G ? action_ptr(h, b, t) : none;
+      const double* ap = c.G ? action_ptr(h, b, ts + t - 1) : none;
+      const double* ac = c.G ? action_ptr(h, b, ts + t) : none;
       step(c, e.sc, e.pm, e.cur, ap, ac, w);
       if (stride > 0 && (t + 1) % stride == 0) e.ckpt.push_back(e.cur);
       if (record) e.rec.push_back(e.cur);
@@ -240,6 +264,7 @@ int32_t oracle_backward(oracle_sim* h, const double* gxT, const double* gvT, dou
                         double* g_material /* [B][5] */) {
   const Config& c = h->c; const int N = c.N, E = c.E(), G = c.G, H = h->H_done, stride = h->stride;
   if (stride <= 0 || H <= 0) return -2;
+  const int ts = h->t_start;   // frames are ts + t; g_actions is indexed by t (relative to the rollout's start)
   if (g_actions) std::memset(g_actions, 0, sizeof(double) * (size_t)H * h->B * G * 6);
 #pragma omp parallel for schedule(dynamic)
   for (int b = 0; b < h->B; ++b) {
@@ -261,7 +286,7 @@ int32_t oracle_backward(oracle_sim* h, const double* gxT, const double* gvT, dou
       State<double> s = e.ckpt[g];
       for (int t = t0; t < t1; ++t) {
         starts.push_back(s);
-        step(c, e.sc, e.pm, s, G ? action_ptr(h, b, t - 1) : none, G ? action_ptr(h, b, t) : none, wd);
+        step(c, e.sc, e.pm, s, G ? action_ptr(h, b, ts + t - 1) : none, G ? action_ptr(h, b, ts + t) : none, wd);
       }
       for (int t = t1 - 1; t >= t0; --t) {
         tape.clear();
@@ -272,7 +297,7 @@ int32_t oracle_backward(oracle_sim* h, const double* gxT, const double* gvT, dou
         for (int j = 0; j < E; ++j) sa.d1[j] = mkv(AD::variable(s0.d1[j].x), AD::variable(s0.d1[j].y), AD::variable(s0.d1[j].z));
         for (int i = 0; i < N; ++i) { sa.k1[i] = AD::variable(s0.k1[i]); sa.k2[i] = AD::variable(s0.k2[i]); }
         std::vector<AD> ap(G ? 6 * G : 1), ac(G ? 6 * G : 1);
-        for (int q = 0; q < 6 * G; ++q) { ap[q] = AD::variable(action_ptr(h, b, t - 1)[q]); ac[q] = AD::variable(action_ptr(h, b, t)[q]); }
+        for (int q = 0; q < 6 * G; ++q) { ap[q] = AD::variable(action_ptr(h, b, ts + t - 1)[q]); ac[q] = AD::variable(action_ptr(h, b, ts + t)[q]); }
         Params<AD> pa;
         pa.stretch = AD::variable(e.pm.stretch); pa.alpha = AD::variable(e.pm.alpha); pa.gamma = AD::variable(e.pm.gamma);
         pa.sigma_y = AD::variable(e.pm.sigma_y); pa.r_c = AD::variable(e.pm.r_c);

@@ -111,6 +111,13 @@ class OracleSim:
         kb = None if kappa_bar0 is None else _d(kappa_bar0)
         lib().oracle_set_state(self.h, _ptr(_d(x0)), _ptr(_d(v0)), _ptr(kb))
 
+    def restore(self, state, t_start):
+        """Harness plumbing: put a full state dict (x, v, d1, kappa_bar as state() returns them) back as the start of
+        the next rollout, which then runs frames t_start, t_start+1, ... (no A0; g_actions of backward() is indexed
+        from t_start)."""
+        lib().oracle_restore_state(self.h, _ptr(_d(state["x"])), _ptr(_d(state["v"])), _ptr(_d(state["d1"])),
+                                   _ptr(_d(state["kappa_bar"])), C.c_int32(int(t_start)))
+
     def rollout(self, horizon=None, stride=None, record=False):
         H = self.H if horizon is None else int(horizon)
         s = self.stride if stride is None else int(stride)

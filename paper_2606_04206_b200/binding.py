@@ -11,10 +11,10 @@ import numpy as np
 from . import build as _build
 
 _F = C.c_float
-EXPORTS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_primitives", "dlo_set_grippers", "dlo_set_state",
-           "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_backward", "dlo_rollout_forward_host",
-           "dlo_backward_host", "dlo_check_numerics", "dlo_scratch_bytes", "dlo_launch_count", "dlo_last_error",
-           "dlo_version")
+STATUS_CALLS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_primitives", "dlo_set_grippers", "dlo_set_state",
+                "dlo_restore_state", "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_backward",
+                "dlo_get_state_adjoint", "dlo_rollout_forward_host", "dlo_backward_host", "dlo_check_numerics")
+EXPORTS = STATUS_CALLS + ("dlo_scratch_bytes", "dlo_launch_count", "dlo_last_error", "dlo_version")
 MATERIAL_KEYS = ("mass_per_vertex", "rest_edge_len", "stretch", "bend_stiffness", "damping", "yield_curv",
                  "creep_rate", "mu_rigid", "mu_self")
 STATUS = {0: "DLO_OK", -1: "DLO_ERR_INVALID_ARG", -2: "DLO_ERR_BAD_STATE", -3: "DLO_ERR_CUDA", -4: "DLO_ERR_OOM",
@@ -55,7 +55,7 @@ def lib():
         L.dlo_scratch_bytes.restype = C.c_size_t
         L.dlo_launch_count.restype = C.c_int64
         L.dlo_launch_count.argtypes = [C.c_void_p]
-        for name in EXPORTS[:13]:
+        for name in STATUS_CALLS:
             getattr(L, name).restype = C.c_int32
         _lib = L
     return _lib
@@ -118,6 +118,14 @@ def dlo_set_grippers(h, init_pose, finger_geom, grasp_verts):
 
 def dlo_set_state(h, x0, v0, kappa_bar0=None):
     _chk(lib().dlo_set_state(h, _p(x0), _p(v0), _p(kappa_bar0)))
+
+
+def dlo_restore_state(h, x, v, d1, kappa_bar, step_index):
+    _chk(lib().dlo_restore_state(h, _p(x), _p(v), _p(d1), _p(kappa_bar), C.c_int32(step_index)))
+
+
+def dlo_get_state_adjoint(h, g_x=None, g_v=None, g_d1=None, g_kappa_bar=None):
+    _chk(lib().dlo_get_state_adjoint(h, _p(g_x), _p(g_v), _p(g_d1), _p(g_kappa_bar)))
 
 
 def dlo_set_actions(h, actions, horizon):
@@ -221,6 +229,31 @@ class DloSim:
         self.x0, self.v0 = self._up(x0), self._up(v0)
         self.kb0 = None if kappa_bar0 is None else self._up(kappa_bar0)
         dlo_set_state(self.h, self.x0, self.v0, self.kb0)
+
+    def restore(self, state, step_index):
+        """exact restore of a state dict (x, v, d1, kappa_bar: numpy or device tensors) as the start of the next rollout"""
+        t = {k: (state[k] if hasattr(state[k], "data_ptr") else self._up(state[k])) for k in ("x", "v", "d1", "kappa_bar")}
+        self._restored = t
+        dlo_restore_state(self.h, t["x"], t["v"], t["d1"], t["kappa_bar"], int(step_index))
+
+    def state_device(self):
+        """current state as fp32 device tensors (no host copy)"""
+        torch = self.torch
+        B, N = self.B, self.N
+        out = {"x": torch.empty((B, 3, N), device=self.dev), "v": torch.empty((B, 3, N), device=self.dev),
+               "d1": torch.empty((B, 3, N), device=self.dev), "kappa_bar": torch.empty((B, 2, N), device=self.dev)}
+        dlo_get_state(self.h, out["x"], out["v"], out["d1"], out["kappa_bar"])
+        return out
+
+    def state_adjoint(self):
+        """adjoint of the rollout's whole start state after backward() (g_x, g_v, g_d1, g_kappa_bar)"""
+        torch = self.torch
+        B, N = self.B, self.N
+        out = {"g_x": torch.empty((B, 3, N), device=self.dev), "g_v": torch.empty((B, 3, N), device=self.dev),
+               "g_d1": torch.empty((B, 3, N), device=self.dev), "g_kappa_bar": torch.empty((B, 2, N), device=self.dev)}
+        dlo_get_state_adjoint(self.h, out["g_x"], out["g_v"], out["g_d1"], out["g_kappa_bar"])
+        torch.cuda.synchronize(self.dev)
+        return {k: t.double().cpu().numpy() for k, t in out.items()}
 
     def rollout(self, horizon=None, stride=None):
         H = self.H if horizon is None else int(horizon)

@@ -52,14 +52,30 @@ struct dlo_sim {
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
   int H_actions = 0, H_done = 0, stride = 0;
-  int tape_seg = -1;               // segment whose tape records are in the buffer already (written by the forward rollout)
-  bool have_state = false, have_prims = false, have_grippers = false;
+  int tape_seg = -1, tape_buf = 0;  // segment whose tape records are in a buffer already (written by the forward rollout), and which buffer
+  int device = 0;                  // the CUDA device the handle was created on (every call must be made with it current)
+  int t_start = 0;                 // frame index of state0 (0 after dlo_set_state; dlo_restore_state sets it)
+  bool have_state = false, have_q = false, have_prims = false, have_grippers = false, have_adj = false;
   int64_t launches = 0;
-  // staging for the *_host calls
-  float *hx0 = nullptr, *hv0 = nullptr, *hkb = nullptr, *hact = nullptr, *hseed_x = nullptr, *hseed_v = nullptr;
-  float *hg_act = nullptr, *hg_x0 = nullptr, *hg_v0 = nullptr, *hg_mat = nullptr, *hxT = nullptr, *hvT = nullptr;
-  int hact_H = 0;
+  // staging of the *_host calls, owned by the handle: pinned host buffers and their device twins
+  float *hx0 = nullptr, *hv0 = nullptr, *hkb = nullptr, *hact = nullptr, *hxT = nullptr, *hvT = nullptr;
+  float *dx0 = nullptr, *dv0 = nullptr, *dkb = nullptr, *dact = nullptr, *dxT = nullptr, *dvT = nullptr;
+  float *dsx = nullptr, *dsv = nullptr, *dga = nullptr, *dgx = nullptr, *dgv = nullptr, *dgm = nullptr;
+  size_t hact_n = 0, dact_n = 0, dga_n = 0;
 };
+
+// every entry point: the handle's device must be the current one
+static dlo_status check_device(const dlo_sim* s) {
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); return fail(DLO_ERR_CUDA, "cudaGetDevice failed"); }
+  if (d != s->device) return fail(DLO_ERR_BAD_STATE, "the handle was created on CUDA device " + std::to_string(s->device) + " but device " + std::to_string(d) + " is current");
+  return DLO_OK;
+}
+#define ENTER(s)                                                       \
+  do {                                                                 \
+    if (!(s)) return fail(DLO_ERR_INVALID_ARG, "NULL handle");         \
+    if (dlo_status st_ = check_device(s)) return st_;                  \
+  } while (0)
 
 static int vpl_for(int N) { return 2 * ((N + 63) / 64); }
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
@@ -177,6 +193,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   dlo_sim* s = new dlo_sim();
   s->cfg = *cfg;
   s->stream = (cudaStream_t)stream;
+  if (cudaGetDevice(&s->device) != cudaSuccess) { cudaGetLastError(); delete s; return fail(DLO_ERR_CUDA, "cudaGetDevice failed"); }
   fill_params(*cfg, s->P);
   KParams& P = s->P;
   s->VPL = vpl_for(P.N);
@@ -190,7 +207,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
     // forward: two CTAs per SM; choose the CTA size whose slots (2 * n_SM * warps) split the batch into whole waves
     // (4096 envs on 148 SMs: 7 warps -> 1.98 waves, where 8 warps would leave the second wave 27 % empty)
     int n_sm = 148;
-    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, s->device);
     // CTA shape: c warps per CTA, as many CTAs per SM as the register file (16 warps at 128 registers) and shared memory allow.  Cost model
     // fitted to a sweep on config 5: time ~ waves * sqrt(warps per SM), larger CTAs slightly
     // better at equal occupancy (more warps share each instruction-cache fill).
@@ -249,14 +266,20 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
 
 dlo_status dlo_destroy(dlo_sim* s) {
   if (!s) return DLO_OK;
+  int cur = -1;
+  cudaGetDevice(&cur);
+  if (cur != s->device) cudaSetDevice(s->device);   // free on the handle's own device, whatever is current
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
                  s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->side[0], s->side[1], s->side_count[0], s->side_count[1], s->tape_slot[0], s->tape_slot[1], s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
   for (void* p : dev) if (p) cudaFree(p);
   if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
   for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
-  void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hseed_x, s->hseed_v, s->hg_act, s->hg_x0, s->hg_v0, s->hg_mat, s->hxT, s->hvT};
+  void* stg[] = {s->dx0, s->dv0, s->dkb, s->dact, s->dxT, s->dvT, s->dsx, s->dsv, s->dga, s->dgx, s->dgv, s->dgm};
+  for (void* p : stg) if (p) cudaFree(p);
+  void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hxT, s->hvT};
   for (void* p : host) if (p) cudaFreeHost(p);
+  if (cur >= 0 && cur != s->device) cudaSetDevice(cur);
   delete s;
   return DLO_OK;
 }
@@ -266,18 +289,19 @@ static dlo_status rebuild_kin(dlo_sim* s) {
   k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->kin);
   s->launches += 1;
   CU(cudaGetLastError());
-  s->have_state = false;
+  s->have_state = false; s->have_q = false;
   return DLO_OK;
 }
 
 dlo_status dlo_set_pins(dlo_sim* s, const uint8_t* pinned) {
-  if (!s || !pinned) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  ENTER(s);
+  if (!pinned) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
   CU(cudaMemcpyAsync(s->pins, pinned, (size_t)s->P.B * s->P.N, cudaMemcpyDeviceToDevice, s->stream));
   return rebuild_kin(s);
 }
 
 dlo_status dlo_set_primitives(dlo_sim* s, const int32_t* types, const float* params) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (s->P.K == 0) return DLO_OK;
   if (!types || !params) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
   for (int k = 0; k < s->P.K; ++k) {
@@ -290,7 +314,7 @@ dlo_status dlo_set_primitives(dlo_sim* s, const int32_t* types, const float* par
 }
 
 dlo_status dlo_set_grippers(dlo_sim* s, const float* init_pose, const float* finger_geom, const int32_t* grasp_verts) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (s->P.G == 0) return DLO_OK;
   if (!init_pose || !finger_geom || !grasp_verts) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
   const size_t BG = (size_t)s->P.B * s->P.G;
@@ -302,7 +326,8 @@ dlo_status dlo_set_grippers(dlo_sim* s, const float* init_pose, const float* fin
 }
 
 dlo_status dlo_set_state(dlo_sim* s, const float* x0, const float* v0, const float* kb0) {
-  if (!s || !x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  ENTER(s);
+  if (!x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
   const KParams& P = s->P;
   if (P.K > 0 && !s->have_prims) return fail(DLO_ERR_BAD_STATE, "dlo_set_primitives must precede dlo_set_state");
   if (P.G > 0 && !s->have_grippers) return fail(DLO_ERR_BAD_STATE, "dlo_set_grippers must precede dlo_set_state");
@@ -314,13 +339,29 @@ dlo_status dlo_set_state(dlo_sim* s, const float* x0, const float* v0, const flo
   CU(cudaGetLastError());
   CU(cudaMemcpyAsync(s->state, s->state0, (size_t)P.B * s->blk * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
   CU(cudaMemsetAsync(s->flags, 0, (size_t)P.B * sizeof(int), s->stream));
-  s->have_state = true;
-  s->H_done = 0; s->stride = 0;
+  s->have_state = true; s->have_q = true; s->have_adj = false;
+  s->H_done = 0; s->stride = 0; s->t_start = 0;
+  return DLO_OK;
+}
+
+dlo_status dlo_restore_state(dlo_sim* s, const float* x, const float* v, const float* d1, const float* kb, int32_t step_index) {
+  ENTER(s);
+  if (!x || !v || !d1 || !kb) return fail(DLO_ERR_INVALID_ARG, "NULL argument (x, v, d1 and kappa_bar are all required)");
+  if (step_index < 0) return fail(DLO_ERR_INVALID_ARG, "step_index < 0");
+  if (!s->have_q) return fail(DLO_ERR_BAD_STATE, "dlo_restore_state needs an earlier dlo_set_state on this scene (grasp-local coordinates are captured there)");
+  const KParams& P = s->P;
+  const size_t n = (size_t)P.B * s->blk;
+  k_put_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, x, v, d1, kb, s->state0);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(s->state, s->state0, n * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  s->have_state = true; s->have_adj = false;
+  s->H_done = 0; s->stride = 0; s->t_start = step_index;
   return DLO_OK;
 }
 
 dlo_status dlo_set_actions(dlo_sim* s, const float* actions, int32_t horizon) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (horizon < 0) return fail(DLO_ERR_INVALID_ARG, "horizon < 0");
   if (s->P.G > 0 && horizon > 0 && !actions) return fail(DLO_ERR_INVALID_ARG, "actions is NULL");
   s->actions = actions; s->H_actions = horizon; s->P.actions = actions;
@@ -431,10 +472,12 @@ static dlo_status ensure_tape(dlo_sim* s, int H, int stride) {
 extern "C" {
 
 dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "dlo_set_state has not been called (or the scene changed since)");
   if (horizon < 0 || stride < 0) return fail(DLO_ERR_INVALID_ARG, "horizon < 0 or checkpoint_stride < 0");
-  if (s->P.G > 0 && horizon > s->H_actions) return fail(DLO_ERR_INVALID_ARG, "horizon exceeds the actions given to dlo_set_actions");
+  if (s->P.G > 0 && s->t_start + horizon > s->H_actions) return fail(DLO_ERR_INVALID_ARG, "start frame + horizon exceeds the actions given to dlo_set_actions");
+  s->P.t_base = s->t_start;
+  s->have_adj = false;
   const KParams& P = s->P;
   const size_t blk_bytes = s->blk * sizeof(float) * P.B;
   CU(cudaMemcpyAsync(s->state, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));
@@ -474,14 +517,14 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     }
     CU(launch_forward(s, Pf, t_last, horizon, stride, true, s->stream));
     s->stat_rep_valid[buf] = s->sort_mode != 0;
-    s->tape_seg = nseg - 1;
+    s->tape_seg = nseg - 1; s->tape_buf = buf;
   } else if (horizon > 0) CU(forward_chunks(s, 0, horizon, stride));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;
 }
 
 dlo_status dlo_get_state(dlo_sim* s, float* x, float* v, float* d1, float* kb) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "no state");
   const KParams& P = s->P;
   const size_t n = (size_t)P.B * STATE_ROWS * P.N;
@@ -492,7 +535,7 @@ dlo_status dlo_get_state(dlo_sim* s, float* x, float* v, float* d1, float* kb) {
 }
 
 dlo_status dlo_check_numerics(dlo_sim* s, int32_t* n_bad) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   std::vector<int> f(s->P.B);
   CU(cudaMemcpyAsync(f.data(), s->flags, f.size() * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));

@@ -24,20 +24,20 @@ static cudaError_t launch_adjoint(dlo_sim* s, const KParams& P, int t0, int t1) 
 extern "C" {
 
 dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g_actions, float* g_x0, float* g_v0, float* g_material) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
   const int H = s->H_done, stride = s->stride, B = s->P.B;
-  const size_t blk = s->blk, rec = (size_t)tape_rows(s->P.N_C) * s->P.NS, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub + 1;
+  const size_t blk = s->blk;
   {
     dlo_status st = ensure_tape(s, H, stride);
     if (st) return st;
   }
-  if (!s->adj) {
-    CU(dalloc(&s->adj, (size_t)B * blk));
-    CU(dalloc(&s->replay, (size_t)B * blk));
-    CU(dalloc(&s->gmat, (size_t)B * 5));
-    if (s->P.self_contact) CU(dalloc(&s->acc_tape, (size_t)B * s->P.N_C * 3 * 33 * s->VPL));
-  }
+  s->have_adj = false;
+  // each buffer on its own: a failed allocation leaves the others (and the handle) usable, and is retried by the next call
+  if (!s->adj) CU(dalloc(&s->adj, (size_t)B * blk));
+  if (!s->replay) CU(dalloc(&s->replay, (size_t)B * blk));
+  if (!s->gmat) CU(dalloc(&s->gmat, (size_t)B * 5));
+  if (s->P.self_contact && !s->acc_tape) CU(dalloc(&s->acc_tape, (size_t)B * s->P.N_C * 3 * 33 * s->VPL));
   const size_t nadj = (size_t)B * blk;
   k_seed_adjoint<<<(unsigned)((nadj + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, gxT, gvT, s->adj);
   s->launches += 1;
@@ -80,6 +80,9 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaStreamWaitEvent(s->aux, s->ev_fwd, 0));
   }
   dlo_status rst = DLO_OK;
+  // the forward rollout chose the buffer of the last segment with the buffers it had THEN; if the set has changed since
+  // (a second tape buffer that could not be allocated before, or was lost), its records are not where this pass looks
+  if (s->tape_seg == nseg - 1 && s->tape_buf != (overlap ? ((nseg - 1) & 1) : 0)) s->tape_seg = -1;
   if (s->tape_seg != nseg - 1 && (rst = replay(nseg - 1))) return rst;     // normally the forward rollout left it on the tape
   const bool have_last = s->tape_seg == nseg - 1;
   s->tape_seg = -1;
@@ -111,47 +114,66 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaGetLastError());
   }
   if (g_material) CU(cudaMemcpyAsync(g_material, s->gmat, (size_t)B * 5 * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
+  s->have_adj = true;
   return DLO_OK;
 }
 
-static dlo_status stage(float** pinned, size_t n) {
+dlo_status dlo_get_state_adjoint(dlo_sim* s, float* g_x, float* g_v, float* g_d1, float* g_kb) {
+  ENTER(s);
+  if (!s->have_adj) return fail(DLO_ERR_BAD_STATE, "dlo_get_state_adjoint needs a completed dlo_backward");
+  const size_t n = (size_t)s->P.B * STATE_ROWS * s->P.N;
+  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->P.B, s->P.N, s->P.NS, s->adj, g_x, g_v, g_d1, g_kb);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  return DLO_OK;
+}
+
+// staging of the *_host calls lives in the handle: grow-only buffers, freed by dlo_destroy
+static dlo_status stage_host(float** pinned, size_t n) {
   if (*pinned) { cudaFreeHost(*pinned); *pinned = nullptr; }
   CU(cudaMallocHost((void**)pinned, (n ? n : 1) * sizeof(float)));
+  return DLO_OK;
+}
+static dlo_status stage_dev(dlo_sim* s, float** p, size_t n) {
+  if (*p) { CU(cudaStreamSynchronize(s->stream)); cudaFree(*p); *p = nullptr; }
+  CU(dalloc(p, n));
   return DLO_OK;
 }
 
 dlo_status dlo_rollout_forward_host(dlo_sim* s, const float* x0, const float* v0, const float* kb0, const float* actions,
                                     int32_t horizon, int32_t stride, float* x_T, float* v_T) {
-  if (!s || !x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  ENTER(s);
+  if (!x0 || !v0) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  if (horizon < 0 || stride < 0) return fail(DLO_ERR_INVALID_ARG, "horizon < 0 or checkpoint_stride < 0");
   const KParams& P = s->P;
   const size_t nx = (size_t)P.B * 3 * P.N, nk = (size_t)P.B * 2 * P.N, na = (size_t)horizon * P.B * P.G * 6;
   if (P.G > 0 && horizon > 0 && !actions) return fail(DLO_ERR_INVALID_ARG, "actions is NULL");
   dlo_status st;
-  if (!s->hx0) { if ((st = stage(&s->hx0, nx))) return st; if ((st = stage(&s->hv0, nx))) return st; if ((st = stage(&s->hkb, nk))) return st;
-                 if ((st = stage(&s->hxT, nx))) return st; if ((st = stage(&s->hvT, nx))) return st; }
-  if (na > 0 && horizon > s->hact_H) { if ((st = stage(&s->hact, na))) return st; s->hact_H = horizon; }
-  // device staging lives in the tail of the same allocations (cudaMallocHost memory is device-accessible only via
-  // copies here): device copies of the inputs
-  static thread_local float *dx0 = nullptr, *dv0 = nullptr, *dkb = nullptr, *dact = nullptr, *dxT = nullptr, *dvT = nullptr;
-  static thread_local size_t dact_n = 0, dx_n = 0;
-  if (dx_n < nx) {
-    cudaFree(dx0); cudaFree(dv0); cudaFree(dkb); cudaFree(dxT); cudaFree(dvT);
-    CU(dalloc(&dx0, nx)); CU(dalloc(&dv0, nx)); CU(dalloc(&dkb, nk)); CU(dalloc(&dxT, nx)); CU(dalloc(&dvT, nx));
-    dx_n = nx;
+  {   // the fixed-size buffers (sizes depend on the config only), each checked on its own
+    float** hp[] = {&s->hx0, &s->hv0, &s->hxT, &s->hvT};
+    float** dp[] = {&s->dx0, &s->dv0, &s->dxT, &s->dvT};
+    for (int k = 0; k < 4; ++k) { if (!*hp[k] && (st = stage_host(hp[k], nx))) return st; if (!*dp[k] && (st = stage_dev(s, dp[k], nx))) return st; }
   }
-  if (dact_n < na) { CU(cudaStreamSynchronize(s->stream)); cudaFree(dact); CU(dalloc(&dact, na)); dact_n = na; }
+  if (!s->hkb && (st = stage_host(&s->hkb, nk))) return st;
+  if (!s->dkb && (st = stage_dev(s, &s->dkb, nk))) return st;
+  if (na > s->hact_n) { if ((st = stage_host(&s->hact, na))) { s->hact_n = 0; return st; } s->hact_n = na; }
+  if (na > s->dact_n) {
+    if (s->actions == s->dact) { s->actions = nullptr; s->P.actions = nullptr; s->H_actions = 0; }   // about to be freed
+    if ((st = stage_dev(s, &s->dact, na))) { s->dact_n = 0; return st; }
+    s->dact_n = na;
+  }
   memcpy(s->hx0, x0, nx * sizeof(float));
   memcpy(s->hv0, v0, nx * sizeof(float));
-  CU(cudaMemcpyAsync(dx0, s->hx0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
-  CU(cudaMemcpyAsync(dv0, s->hv0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
-  if (kb0) { memcpy(s->hkb, kb0, nk * sizeof(float)); CU(cudaMemcpyAsync(dkb, s->hkb, nk * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
-  if (na > 0) { memcpy(s->hact, actions, na * sizeof(float)); CU(cudaMemcpyAsync(dact, s->hact, na * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
-  if ((st = dlo_set_state(s, dx0, dv0, kb0 ? dkb : nullptr))) return st;
-  if ((st = dlo_set_actions(s, dact, horizon))) return st;
+  CU(cudaMemcpyAsync(s->dx0, s->hx0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  CU(cudaMemcpyAsync(s->dv0, s->hv0, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  if (kb0) { memcpy(s->hkb, kb0, nk * sizeof(float)); CU(cudaMemcpyAsync(s->dkb, s->hkb, nk * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
+  if (na > 0) { memcpy(s->hact, actions, na * sizeof(float)); CU(cudaMemcpyAsync(s->dact, s->hact, na * sizeof(float), cudaMemcpyHostToDevice, s->stream)); }
+  if ((st = dlo_set_state(s, s->dx0, s->dv0, kb0 ? s->dkb : nullptr))) return st;
+  if ((st = dlo_set_actions(s, s->dact, horizon))) return st;   // the handle's own copy: stays valid for dlo_backward
   if ((st = dlo_rollout_forward(s, horizon, stride))) return st;
-  if ((st = dlo_get_state(s, x_T ? dxT : nullptr, v_T ? dvT : nullptr, nullptr, nullptr))) return st;
-  if (x_T) CU(cudaMemcpyAsync(s->hxT, dxT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
-  if (v_T) CU(cudaMemcpyAsync(s->hvT, dvT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if ((st = dlo_get_state(s, x_T ? s->dxT : nullptr, v_T ? s->dvT : nullptr, nullptr, nullptr))) return st;
+  if (x_T) CU(cudaMemcpyAsync(s->hxT, s->dxT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (v_T) CU(cudaMemcpyAsync(s->hvT, s->dvT, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
   if (x_T) memcpy(x_T, s->hxT, nx * sizeof(float));
   if (v_T) memcpy(v_T, s->hvT, nx * sizeof(float));
@@ -159,24 +181,24 @@ dlo_status dlo_rollout_forward_host(dlo_sim* s, const float* x0, const float* v0
 }
 
 dlo_status dlo_backward_host(dlo_sim* s, const float* gxT, const float* gvT, float* g_actions, float* g_x0, float* g_v0, float* g_material) {
-  if (!s) return fail(DLO_ERR_INVALID_ARG, "NULL handle");
+  ENTER(s);
   if (s->stride <= 0 || s->H_done <= 0) return fail(DLO_ERR_BAD_STATE, "dlo_backward needs a rollout with checkpoint_stride > 0");
   const KParams& P = s->P;
   const size_t nx = (size_t)P.B * 3 * P.N, na = (size_t)s->H_done * P.B * P.G * 6, nm = (size_t)P.B * DLO_N_MATERIAL_GRADS;
-  static thread_local float *dsx = nullptr, *dsv = nullptr, *dga = nullptr, *dgx = nullptr, *dgv = nullptr, *dgm = nullptr;
-  static thread_local size_t nx_a = 0, na_a = 0, nm_a = 0;
-  if (nx_a < nx) { cudaFree(dsx); cudaFree(dsv); cudaFree(dgx); cudaFree(dgv); CU(dalloc(&dsx, nx)); CU(dalloc(&dsv, nx)); CU(dalloc(&dgx, nx)); CU(dalloc(&dgv, nx)); nx_a = nx; }
-  if (na_a < na) { cudaFree(dga); CU(dalloc(&dga, na)); na_a = na; }
-  if (nm_a < nm) { cudaFree(dgm); CU(dalloc(&dgm, nm)); nm_a = nm; }
-  if (gxT) CU(cudaMemcpyAsync(dsx, gxT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
-  if (gvT) CU(cudaMemcpyAsync(dsv, gvT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
-  dlo_status st = dlo_backward(s, gxT ? dsx : nullptr, gvT ? dsv : nullptr, (g_actions && na) ? dga : nullptr, g_x0 ? dgx : nullptr,
-                               g_v0 ? dgv : nullptr, g_material ? dgm : nullptr);
+  dlo_status st;
+  float** dp[] = {&s->dsx, &s->dsv, &s->dgx, &s->dgv};
+  for (float** q : dp) if (!*q && (st = stage_dev(s, q, nx))) return st;
+  if (!s->dgm && (st = stage_dev(s, &s->dgm, nm))) return st;
+  if (na > s->dga_n) { if ((st = stage_dev(s, &s->dga, na))) { s->dga_n = 0; return st; } s->dga_n = na; }
+  if (gxT) CU(cudaMemcpyAsync(s->dsx, gxT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  if (gvT) CU(cudaMemcpyAsync(s->dsv, gvT, nx * sizeof(float), cudaMemcpyHostToDevice, s->stream));
+  st = dlo_backward(s, gxT ? s->dsx : nullptr, gvT ? s->dsv : nullptr, (g_actions && na) ? s->dga : nullptr, g_x0 ? s->dgx : nullptr,
+                    g_v0 ? s->dgv : nullptr, g_material ? s->dgm : nullptr);
   if (st) return st;
-  if (g_actions && na) CU(cudaMemcpyAsync(g_actions, dga, na * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
-  if (g_x0) CU(cudaMemcpyAsync(g_x0, dgx, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
-  if (g_v0) CU(cudaMemcpyAsync(g_v0, dgv, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
-  if (g_material) CU(cudaMemcpyAsync(g_material, dgm, nm * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_actions && na) CU(cudaMemcpyAsync(g_actions, s->dga, na * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_x0) CU(cudaMemcpyAsync(g_x0, s->dgx, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_v0) CU(cudaMemcpyAsync(g_v0, s->dgv, nx * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
+  if (g_material) CU(cudaMemcpyAsync(g_material, s->dgm, nm * sizeof(float), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
   return DLO_OK;
 }

@@ -124,6 +124,21 @@ __global__ void k_get_state(int B, int N, int NS, const float* state, float* x, 
   else if (kb) kb[((size_t)env * 2 + q - 9) * N + i] = val;
 }
 
+// user arrays -> internal state block (exact restore: the inverse of k_get_state; padding columns zeroed)
+__global__ void k_put_state(int B, int N, int NS, const float* x, const float* v, const float* d1, const float* kb, float* state) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)B * STATE_ROWS * NS) return;
+  const int i = (int)(idx % NS), q = (int)((idx / NS) % STATE_ROWS), env = (int)(idx / ((size_t)NS * STATE_ROWS));
+  float val = 0.0f;
+  if (i < N) {
+    if (q < 3) val = x[((size_t)env * 3 + q) * N + i];
+    else if (q < 6) val = v[((size_t)env * 3 + q - 3) * N + i];
+    else if (q < 9) val = d1[((size_t)env * 3 + q - 6) * N + i];
+    else val = kb[((size_t)env * 2 + q - 9) * N + i];
+  }
+  state[idx] = val;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // per-warp start-up shared by the forward and adjoint kernels: primitives (boxes expanded to rotation
 // matrices), grasp-local coordinates, zeroed accumulators
@@ -156,8 +171,9 @@ __device__ __forceinline__ void warp_setup(const KParams& P, int env, int lane, 
 
 __device__ __forceinline__ void load_actions(const KParams& P, int env, int lane, int t, float ap[6], float ac[6]) {
   if (lane < P.G) {
-    const float* cur = P.actions + (((size_t)t * P.B + env) * P.G + lane) * 6;
-    const float* prv = (t > 0) ? P.actions + (((size_t)(t - 1) * P.B + env) * P.G + lane) * 6 : P.pose0 + ((size_t)env * P.G + lane) * 6;
+    const int ta = P.t_base + t;   // absolute frame (a rollout restored by dlo_restore_state starts at t_base > 0)
+    const float* cur = P.actions + (((size_t)ta * P.B + env) * P.G + lane) * 6;
+    const float* prv = (ta > 0) ? P.actions + (((size_t)(ta - 1) * P.B + env) * P.G + lane) * 6 : P.pose0 + ((size_t)env * P.G + lane) * 6;
 #pragma unroll
     for (int k = 0; k < 6; ++k) { ap[k] = prv[k]; ac[k] = cur[k]; }
   }

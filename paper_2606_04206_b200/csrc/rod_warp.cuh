@@ -27,6 +27,7 @@ enum { PRIM_NP = 10, PRIM_SM_STRIDE = 20, PRIM_BC = 16, PRIM_BR = 19 };
 struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
   int G, M, K, cand_cap, hot_cap;
+  int t_base;            // frame index of the rollout's first step: step t of the launch uses actions[t_base + t - 1], actions[t_base + t]
   float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
   int vote_mode;         // bit 0: the warps of a CTA refresh their contact data together; bit 1: ... and rebuild their pair lists together
   float near_dist;       // pairs closer than this at a full filter go to the near list (measured every substep)

@@ -100,8 +100,38 @@ def _base(cfg_id, batch, n_verts, horizon, stride):
     return cfg, B, N, H, S
 
 
+FLOAT_CONFIG_KEYS = ("dt", "rope_radius", "contact_softness", "influence_threshold", "restitution")
+ARRAY_KEYS = ("x0", "v0", "kappa_bar0", "prim_params", "init_pose", "finger_geom", "actions")
+
+
+def representable(P):
+    """Rounds every real input of a problem dict to its nearest fp32 value (still stored as float64), so that the fp64
+    oracle and the fp32 library read the SAME numbers.  The step has branches decided at exact thresholds (a vertex
+    resting at phi = r sits on the kink of f = min(exp(d / eps_s), 1)): with r = 2.5e-3 given to one side as
+    a double and to the other as its fp32 rounding, the two would take different sides of every such tie by construction."""
+    f = lambda a: np.asarray(a, dtype=np.float32).astype(np.float64)
+    P = dict(P)
+    cfg = dict(P["config"])
+    for k in FLOAT_CONFIG_KEYS:
+        cfg[k] = float(np.float32(cfg[k]))
+    cfg["gravity"] = tuple(float(np.float32(g)) for g in cfg["gravity"])
+    P["config"] = cfg
+    P["material"] = {k: f(v) for k, v in P["material"].items()}
+    for k in ARRAY_KEYS:
+        if P.get(k) is not None:
+            P[k] = f(P[k])
+    if P.get("loss") is not None:
+        P["loss"] = dict(P["loss"], target=f(P["loss"]["target"]))
+    return P
+
+
 def make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
-    """Problem dict for BASELINE.json config `cfg_id` (1..5); size overrides give the reduced parity cases."""
+    """Problem dict for BASELINE.json config `cfg_id` (1..5); size overrides give the reduced parity cases.  Every real
+    input is fp32-representable (see `representable`)."""
+    return representable(_make_problem(cfg_id, batch, n_verts, horizon, stride))
+
+
+def _make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
     rng = np.random.Generator(np.random.PCG64(SEED0 + cfg_id))
     cfg, B, N, H, S = _base(cfg_id, batch, n_verts, horizon, stride)
     P = dict(config=cfg, horizon=H, checkpoint_stride=S, config_id=cfg_id, pins=None, kappa_bar0=None, actions=None)
