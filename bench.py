@@ -1,15 +1,21 @@
 #!/usr/bin/env python
 """bench.py — env-steps/s of the batched differentiable rod step at BASELINE.json config 5 (4096 ropes x 128 verts).
 
-One "step" of this benchmark = one pass of the whole hot path over one batch of synthetic input: a full
-forward rollout (H frames of 5 substeps, checkpoints every `stride` frames) followed by the checkpointed reverse
-pass (`--mode fwdbwd`, default) or the forward rollout alone (`--mode fwd`).  `value` = B*H*n_gpus / time,
-timed with CUDA events on the launching stream, inputs resident in HBM.  `e2e` is the same metric through the
-host-buffer C-ABI calls (host->device copies of x0, v0, actions and device->host copies of x_T and the
-gradients inside the timed region).  `--impl reference` times the fp64 CPU oracle on a bounded sample instead.
+BASELINE.json's metric is "fwd AND fwd+bwd env-steps/s": one run measures both and prints ONE JSON line.
+  value / ms_per_step   one "step" = one pass of the whole hot path over one batch of synthetic input: a full forward
+                        rollout (H frames of 5 substeps, checkpoints every `stride` frames) followed by the checkpointed
+                        reverse pass.  value = B*H*n_gpus / time, CUDA events on the launching stream, inputs resident in HBM.
+  forward               {value, ms_per_step, roofline}: the forward rollout alone (no checkpoints), timed the same way.
+  e2e                   the fwd+bwd pass through the host-buffer C-ABI calls (host->device copies of x0, v0, actions and
+                        device->host copies of x_T and the gradients inside the timed region).
+  roofline              for the dominant kernel of the fwd+bwd pass (k_adjoint): algorithmic flops of its launches divided by
+                        their durations, measured live with CUDA events on the launching stream (dlo_set_kernel_timing),
+                        against the fp32 peak MEASURED in the same run by the library's FFMA-chain microbenchmark.
+  cpu_baseline          the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0).
+`--impl reference` times the oracle instead (the tier's reference arm).  `--mode fwd|fwdbwd` restricts a run to one mode.
 
-Prints ONE JSON line.  Multi-GPU (torchrun): envs are independent, so ranks run disjoint shards of the batch
-with no collective on the data path ("scaling": "weak"); the time is the max over ranks.
+Multi-GPU (torchrun): envs are independent, so ranks run disjoint shards of the batch with no collective on the data
+path ("scaling": "weak"); every time is the max over ranks.
 """
 import argparse
 import json
@@ -28,16 +34,11 @@ from workloads.configs import make_problem, loss_and_seed, FULL_SIZES  # noqa: E
 
 METRIC = "env_steps_per_s"
 UNIT = "env-steps/s"
-# Algorithmic fp32 flops per env-step of config 5 (5 substeps, N=128, N_C=10, 4 primitives + 4 finger capsules), counted
-# in DESIGN.md section 7 (FADD/FMUL = 1, FFMA = 2): forward 0.10 Mflop per substep = 0.5 Mflop per env-step; the reverse of a
-# substep 0.17 Mflop; forward+backward = forward + replay + reverse = 0.5 + 0.5 + 0.85 = 1.85 Mflop per env-step.
-FLOPS_PER_ENV_STEP = {"fwd": 0.5e6, "fwdbwd": 1.85e6}
-# DRAM bytes per env-substep of the dominant kernel (k_adjoint), from the `ncu --set full` capture summarised in
-# profiles/r01_final_ncu_summary.md: (34.829 GB read + 0.237 GB written) / (4096 envs x 100 frames x 5 substeps) = 17.1 KB,
-# against 16.4 KB of tape record it has to read (algorithmic) plus the side records of the self-contact substeps.
-ADJ_DRAM_BYTES_PER_ENV_SUBSTEP = (34.829228e9 + 0.237290e9) / (4096 * 100 * 5)
-# fp32 ALU peak derived in DESIGN.md section 7: 148 SMs x 128 lanes x 2 flop x 1.965 GHz
-ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# Algorithmic fp32 flops per env-step of config 5 (5 substeps, N=128, N_C=10, 4 primitives + 4 finger capsules), counted in
+# DESIGN.md section 5 (FADD/FMUL = 1, FFMA = 2): forward kernel 0.5 Mflop, the same for the replay, adjoint kernel 0.85 Mflop.
+# They are hand counts for config 5 only: no roofline is printed for another config.
+ALG_FLOPS = {"k_forward": 0.5e6, "k_replay": 0.5e6, "k_adjoint": 0.85e6}
+TAPE_ROWS_BASE = 22          # tape record rows besides the N_C multiplier rows (rod_warp.cuh: 14 state, dx 3, v1 3, S, mask)
 
 
 class ClockSampler(threading.Thread):
@@ -79,7 +80,8 @@ def measured_peaks():
 
 
 def oracle_leg(problem, mode, budget_s, steps=1, warmup=0):
-    """the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, host cores)"""
+    """the fp64 oracle, as it stands, on a bounded sample of the same workload (rank 0, host cores).
+    Returns (cpu_baseline dict, seconds per pass, passes actually timed)."""
     from oracle import dlo_oracle as orc
     cores = orc.num_threads()
     H_full, stride = problem["horizon"], problem["checkpoint_stride"]
@@ -100,8 +102,8 @@ def oracle_leg(problem, mode, budget_s, steps=1, warmup=0):
     envs = np.arange(min(B, cores))
     probe_H = 4
     rate = len(envs) * probe_H / one(envs, probe_H)          # env-steps/s, rough
-    # size the sample for ~budget_s/2 per pass: grow the horizon first, then the number of envs
-    units = max(rate * budget_s * 0.5, len(envs) * probe_H)
+    # size one pass for ~budget_s / (passes + 1): grow the horizon first, then the number of envs
+    units = max(rate * budget_s / (steps + warmup + 1), len(envs) * probe_H)
     H = int(min(H_full, max(probe_H, units // len(envs))))
     n_env = int(min(B, max(len(envs), (units // H) // cores * cores)))
     envs = np.arange(n_env)
@@ -110,12 +112,10 @@ def oracle_leg(problem, mode, budget_s, steps=1, warmup=0):
         dt = one(envs, H)
         if it >= warmup:
             times.append(dt)
-        if sum(times) > budget_s:
-            break
     t = float(np.mean(times))
     return {"value": len(envs) * H / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "%d envs x %d steps of config %d (%s, fp64%s), %.1f s per pass" % (
-                len(envs), H, problem.get("config_id", 5), mode, ", tape-AD reverse" if mode != "fwd" else "", t)}, t, len(envs) * H
+            "sample": "%d envs x %d steps of config %d (%s, fp64%s), %.1f s per pass, %d passes timed" % (
+                len(envs), H, problem.get("config_id", 5), mode, ", tape-AD reverse" if mode != "fwd" else "", t, len(times))}, t, len(times)
 
 
 def main():
@@ -124,7 +124,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--mode", default="fwdbwd", choices=["fwd", "fwdbwd"])
+    ap.add_argument("--mode", default="both", choices=["both", "fwd", "fwdbwd"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--batch", type=int, default=None, help="per-GPU batch (default: the config's)")
     ap.add_argument("--horizon", type=int, default=None)
@@ -138,20 +138,26 @@ def main():
     full = FULL_SIZES[args.config]
     B = args.batch or full["batch"]
     H = args.horizon or full["horizon"]
-    stride = full["stride"] if args.mode == "fwdbwd" else 0
-    workload = "config %d: %d ropes x %d verts per GPU, %d frames x 5 substeps, stride %d" % (args.config, B, full["n_verts"], H, stride)
+    N = full["n_verts"]
+    stride = full["stride"] if full["stride"] > 0 else H      # config 2 is forward-only in BASELINE.json: one segment if asked for a reverse pass
+    stride = min(stride, H)
+    main_mode = "fwd" if args.mode == "fwd" else "fwdbwd"
+    workload = "config %d: %d ropes x %d verts per GPU, %d frames x 5 substeps, checkpoint stride %d" % (args.config, B, N, H, stride)
     base = {"metric": METRIC, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload, "mode": args.mode, "per_gpu_batch": B, "n_verts": full["n_verts"], "horizon": H,
-                       "checkpoint_stride": stride, "cache": "inputs (actions %.0f MB) larger than L2" % (H * B * 2 * 6 * 4 / 1e6)}}
+            "config": {"workload": workload, "mode": main_mode, "per_gpu_batch": B, "n_verts": N, "horizon": H,
+                       "checkpoint_stride": stride if main_mode == "fwdbwd" else 0,
+                       "cache": "inputs (actions %.0f MB) larger than L2" % (H * B * 2 * 6 * 4 / 1e6)}}
 
     if args.impl == "reference":
         if rank != 0:
             return
-        problem = make_problem(args.config, batch=min(B, 256), horizon=H, stride=full["stride"])
-        cb, t, units = oracle_leg(problem, args.mode, budget_s=60, steps=args.steps, warmup=min(args.warmup, 1))
+        problem = make_problem(args.config, batch=min(B, 256), horizon=H, stride=stride)
+        cb, t, n_timed = oracle_leg(problem, main_mode, budget_s=60, steps=args.steps, warmup=min(args.warmup, 1))
         line = dict(base, impl="reference", value=cb["value"], ms_per_step=t * 1e3, dtype="f64", cpu_baseline=cb,
                     e2e={"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, gpu_launches=0)
+        line["steps"] = n_timed
+        line["warmup"] = min(args.warmup, 1)
         line["config"] = dict(line["config"], sample=cb["sample"])
         print(json.dumps(line))
         return
@@ -167,61 +173,86 @@ def main():
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
 
+    # the denominator first, on an idle GPU: fp32 FFMA-chain microbenchmark of the library
+    peak_tf, peak_ms, n_sm = dlo.dlo_measure_fp32_peak(torch.cuda.current_stream().cuda_stream)
+
     # each rank generates its own shard: same recipe, env ids offset by rank (weak scaling, no data-path collective)
     problem = make_problem(args.config, batch=B, horizon=H)
     if world > 1:
         rng = np.random.Generator(np.random.PCG64(977 + rank))
         problem["x0"] = problem["x0"] + rng.normal(0, 1e-5, problem["x0"].shape)
     sim = dlo.DloSim(problem, device=str(dev))
-    seed_t = None
+    G = sim.G
+    target = torch.as_tensor(problem["loss"]["target"], dtype=torch.float32, device=dev)
+    if target.dim() == 2:
+        target = torch.zeros((B, 3, N), device=dev)
+    seed_t, x_t = torch.zeros((B, 3, N), device=dev), torch.empty((B, 3, N), device=dev)
+    grads = {"a": torch.zeros((H, B, max(G, 1), 6), device=dev), "x": torch.zeros((B, 3, N), device=dev),
+             "v": torch.zeros((B, 3, N), device=dev), "m": torch.zeros((B, 5), device=dev)}
 
-    def one_pass():
-        nonlocal seed_t
+    def fwd_pass():
+        dlo.dlo_rollout_forward(sim.h, H, 0)
+
+    def fwdbwd_pass():
         dlo.dlo_rollout_forward(sim.h, H, stride)
-        if args.mode == "fwdbwd":
-            if seed_t is None:
-                seed_t = torch.zeros((B, 3, full["n_verts"]), device=dev)
-                grads = {"a": torch.zeros((H, B, sim.G, 6), device=dev), "x": torch.zeros((B, 3, full["n_verts"]), device=dev),
-                         "v": torch.zeros((B, 3, full["n_verts"]), device=dev), "m": torch.zeros((B, 5), device=dev)}
-                one_pass.grads = grads
-            # loss head of the harness: mean squared distance to the target polyline -> dL/dx_T on the device
-            x = torch.empty_like(seed_t)
-            dlo.dlo_get_state(sim.h, x)
-            seed_t.copy_((x - one_pass.target) * (2.0 / full["n_verts"]))
-            g = one_pass.grads
-            dlo.dlo_backward(sim.h, seed_t, None, g["a"], g["x"], g["v"], g["m"])
-
-    one_pass.target = torch.as_tensor(problem["loss"]["target"], dtype=torch.float32, device=dev)
-    if one_pass.target.dim() == 2:
-        one_pass.target = torch.zeros((B, 3, full["n_verts"]), device=dev)
+        # loss head of the harness: mean squared distance to the target polyline -> dL/dx_T on the device
+        dlo.dlo_get_state(sim.h, x_t)
+        torch.sub(x_t, target, out=seed_t)
+        seed_t.mul_(2.0 / N)
+        dlo.dlo_backward(sim.h, seed_t, None, grads["a"] if G > 0 else None, grads["x"], grads["v"], grads["m"])
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(args.warmup):
-        one_pass()
-    barrier()
-    l0 = dlo.dlo_launch_count(sim.h)
+    def timed(one_pass):
+        """W untimed + K timed passes, barrier + synchronize on both sides, CUDA events, max over ranks"""
+        for _ in range(args.warmup):
+            one_pass()
+        barrier()
+        dlo.dlo_set_kernel_timing(sim.h, True)
+        l0 = dlo.dlo_launch_count(sim.h)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+        ev[0].record()
+        for k in range(args.steps):
+            one_pass()
+            ev[k + 1].record()
+        barrier()
+        launches = dlo.dlo_launch_count(sim.h) - l0
+        kt = [dlo.dlo_get_kernel_timing(sim.h, c) for c in range(3)]
+        dlo.dlo_set_kernel_timing(sim.h, False)
+        per = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
+        ms = max_over_ranks(ev[0].elapsed_time(ev[-1]), dev) / args.steps
+        return {"ms_per_step": ms, "value": B * H * world / (ms * 1e-3), "launches": int(launches), "ms_per_pass": per, "kernels": kt}
+
+    def kernel_roofline(name, kt):
+        """roofline object of one kernel class from its live event timing (config 5 only: the flop counts are config 5's)"""
+        n, tot_ms, units = kt
+        if args.config != 5 or n == 0:
+            return None
+        achieved = ALG_FLOPS[name] * units / (tot_ms * 1e-3) / 1e12
+        r = {"bound": "alu", "kernel": name, "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
+             "launches_timed": n, "ms_per_launch": tot_ms / n, "env_steps_per_launch": units // n,
+             "algorithmic_flops_per_env_step": ALG_FLOPS[name],
+             "peak_source": "measured: FFMA-chain microbenchmark of the library in this run (%d SMs, %.1f ms)" % (n_sm, peak_ms),
+             "traffic": None}
+        if name != "k_forward":
+            # HBM bytes one launch has to move by construction: its tape records (written by the replay, read once by the adjoint)
+            rec_bytes = (TAPE_ROWS_BASE + problem["config"]["n_proj_iters"]) * ((N + 3) // 4 * 4) * 4
+            r["traffic"] = int(units // n * problem["config"]["n_substeps"] * rec_bytes)
+            r["traffic_source"] = "tape layout: (22 + N_C) rows x NS x 4 B per env-substep x the env-substeps of one launch; ncu's dram bytes: profiles/"
+            r["hbm_gbs"] = r["traffic"] / (tot_ms / n * 1e-3) / 1e9
+        return r
+
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    ev[0].record()
-    for k in range(args.steps):
-        one_pass()
-        ev[k + 1].record()
-    barrier()
+    res_fb = timed(fwdbwd_pass) if args.mode in ("both", "fwdbwd") else None
+    res_f = timed(fwd_pass) if args.mode in ("both", "fwd") else None
     clocks = sampler.stop()
-    launches = dlo.dlo_launch_count(sim.h) - l0
-    per = [ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)]
-    total_ms = ev[0].elapsed_time(ev[-1])
-    total_ms = max_over_ranks(total_ms, dev)
     n_bad = sim.n_bad()
-    ms_per_step = total_ms / args.steps
-    value = B * H * world / (ms_per_step * 1e-3)
 
-    # end to end through the host-buffer C-ABI calls
+    # end to end through the host-buffer C-ABI calls (the fwd+bwd pass, or the forward pass in --mode fwd)
     e2e = None
     if not args.no_e2e:
         x0h = np.ascontiguousarray(problem["x0"], dtype=np.float32)
@@ -232,15 +263,15 @@ def main():
         gah, gmh = np.empty_like(acth), np.empty((B, 5), dtype=np.float32)
         h2d = x0h.nbytes + v0h.nbytes + acth.nbytes
         d2h = xTh.nbytes
-
-        def e2e_pass():
-            dlo.dlo_rollout_forward_host(sim.h, x0h, v0h, None, acth, H, stride, xTh, None)
-            if args.mode == "fwdbwd":
-                seed = ((xTh - tgt) * (2.0 / full["n_verts"])).astype(np.float32)
-                dlo.dlo_backward_host(sim.h, seed, None, gah, None, None, gmh)
-        if args.mode == "fwdbwd":
+        if main_mode == "fwdbwd":
             h2d += x0h.nbytes
             d2h += gah.nbytes + gmh.nbytes
+
+        def e2e_pass():
+            dlo.dlo_rollout_forward_host(sim.h, x0h, v0h, None, acth, H, stride if main_mode == "fwdbwd" else 0, xTh, None)
+            if main_mode == "fwdbwd":
+                seed = ((xTh - tgt) * (2.0 / N)).astype(np.float32)
+                dlo.dlo_backward_host(sim.h, seed, None, gah, None, None, gmh)
         e2e_pass()
         barrier()
         t0 = time.perf_counter()
@@ -248,26 +279,29 @@ def main():
         for _ in range(n_e2e):
             e2e_pass()
         barrier()
-        te = (time.perf_counter() - t0) / n_e2e
-        te = max_over_ranks(te, dev)
-        e2e = {"value": B * H * world / te, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+        te = max_over_ranks((time.perf_counter() - t0) / n_e2e, dev)
+        e2e = {"value": B * H * world / te, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "passes_timed": n_e2e}
 
     if rank != 0:
         return
     peaks, which = measured_peaks()
-    flops = FLOPS_PER_ENV_STEP[args.mode] * B * H          # per pass on this GPU (= per launch group)
-    achieved = flops / (min(per) * 1e-3) / 1e12
-    line = dict(base, value=value, ms_per_step=ms_per_step, e2e=e2e, gpu_launches=int(launches), clocks=clocks,
-                roofline={"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / ALU_PEAK_TFLOPS,
-                          "traffic": (ADJ_DRAM_BYTES_PER_ENV_SUBSTEP * B * max(stride, 1) * 5 if args.mode == "fwdbwd" else None),
-                          "traffic_note": "DRAM bytes per k_adjoint launch (one checkpoint segment), ncu capture in profiles/r01_final_ncu_summary.md",
-                          "peak_source": "derived (148 SMs x 128 fp32 lanes x 2 x %.0f MHz, DESIGN.md section 7); HBM peak %s %.0f GB/s" % (
-                              peaks.get("sm_max_mhz", 1965.0), which, peaks.get("hbm_gbs", 0.0)),
-                          "kernel": "k_forward" if args.mode == "fwd" else "k_forward + k_adjoint",
-                          "algorithmic_flops_per_env_step": FLOPS_PER_ENV_STEP[args.mode]},
-                envs_flagged=int(n_bad), ms_per_pass=per)
+    main_res = res_fb if res_fb is not None else res_f
+    line = dict(base, value=main_res["value"], ms_per_step=main_res["ms_per_step"], e2e=e2e, gpu_launches=main_res["launches"], clocks=clocks,
+                envs_flagged=int(n_bad), ms_per_pass=main_res["ms_per_pass"],
+                fp32_peak={"tflops": peak_tf, "source": "FFMA-chain microbenchmark (dlo_measure_fp32_peak), idle GPU, best of 3", "n_sm": n_sm,
+                           "nominal_tflops": n_sm * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12, "hbm_gbs_" + which: peaks.get("hbm_gbs")})
+    if res_fb is not None:
+        line["roofline"] = kernel_roofline("k_adjoint", res_fb["kernels"][2])
+        line["kernel_share"] = {name: {"launches": kt[0], "ms_per_step": kt[1] / args.steps}
+                                for name, kt in zip(("k_forward", "k_replay", "k_adjoint"), res_fb["kernels"])}
+        line["roofline_replay"] = kernel_roofline("k_replay", res_fb["kernels"][1])
+    else:
+        line["roofline"] = kernel_roofline("k_forward", res_f["kernels"][0])
+    if res_f is not None and res_fb is not None:
+        line["forward"] = {"value": res_f["value"], "unit": UNIT, "ms_per_step": res_f["ms_per_step"], "gpu_launches": res_f["launches"],
+                           "ms_per_pass": res_f["ms_per_pass"], "roofline": kernel_roofline("k_forward", res_f["kernels"][0])}
     if not args.no_cpu_baseline:
-        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H, stride=full["stride"]), args.mode, budget_s=20)
+        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H, stride=stride), main_mode, budget_s=20)
         line["cpu_baseline"] = cb
     print(json.dumps(line))
 

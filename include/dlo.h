@@ -14,7 +14,8 @@
  * replayed in reverse (L115).
  *
  * Conventions
- *   - All arithmetic on the GPU is fp32.  B = batch, N = n_verts, E = N-1 (open) or N (ring), G = n_grippers,
+ *   - All arithmetic on the GPU is fp32; vertex positions are carried as an unevaluated sum of two fp32 numbers (x plus
+ *     the residual x_lo that the rounding of x + h v dropped), so that edge vectors are exact differences.  B = batch, N = n_verts, E = N-1 (open) or N (ring), G = n_grippers,
  *     M = n_grasp_max, K = n_primitives, H = horizon (steps = frames).
  *   - Every array argument says "dev" (CUDA device pointer, 16-byte aligned) or "host".  Layouts are dense,
  *     row-major, last index fastest: x, v, d1 are [B][3][N] (SoA per env; d1 uses the first E columns);
@@ -107,18 +108,22 @@ dlo_status dlo_rollout_forward(dlo_sim* sim, int32_t horizon, int32_t checkpoint
 /* Current state; each pointer dev, may be NULL.  x, v, d1: [B][3][N]; kappa_bar: [B][2][N]. */
 dlo_status dlo_get_state(dlo_sim* sim, float* x, float* v, float* d1, float* kappa_bar);
 
+/* Low part of the positions (dev [B][3][N]): the state's positions are x + x_lo with x as dlo_get_state returns them and
+ * |x_lo| <= ulp(x)/2.  Needed only to put a state back EXACTLY (dlo_restore_state). */
+dlo_status dlo_get_position_residual(dlo_sim* sim, float* x_lo);
+
 /* Exact restore (a checkpoint is "a single state"; the segment is re-run from it).  Puts back a
- * state as dlo_get_state returned it, bit for bit: x, v, d1 dev [B][3][N], kappa_bar dev [B][2][N] (all four
- * required), and `step_index`, the frame the next dlo_rollout_forward starts at: its step k uses the actions
+ * state as dlo_get_state (+ dlo_get_position_residual) returned it, bit for bit: x, v, d1 dev [B][3][N], kappa_bar dev
+ * [B][2][N] (all four required), x_lo dev [B][3][N] or NULL (= 0: the positions are then exactly x), and `step_index`, the frame the next dlo_rollout_forward starts at: its step k uses the actions
  * a_{step_index+k-1} -> a_{step_index+k} of the array given to dlo_set_actions (a_{-1} = init_pose), so
  * step_index + horizon must not exceed that array.  No A0 runs: the frames are taken as given, and the grasp-local
  * coordinates stay those captured by the last dlo_set_state (DLO_ERR_BAD_STATE if there was none, or if the scene
- * changed since).  dlo_get_state -> dlo_restore_state -> rollout of k steps equals k more steps of the original
+ * changed since).  dlo_get_state + dlo_get_position_residual -> dlo_restore_state -> rollout of k steps equals k more steps of the original
  * rollout bitwise.  dlo_backward after such a rollout differentiates that segment only: g_actions [horizon][B][G][6]
  * is indexed from step_index (the gradient with respect to a_{step_index-1} is dropped, like that of init_pose),
  * g_x0 / g_v0 are with respect to the restored x, v.  dlo_set_state resets step_index to 0. */
-dlo_status dlo_restore_state(dlo_sim* sim, const float* x, const float* v, const float* d1, const float* kappa_bar,
-                             int32_t step_index);
+dlo_status dlo_restore_state(dlo_sim* sim, const float* x, const float* x_lo, const float* v, const float* d1,
+                             const float* kappa_bar, int32_t step_index);
 
 /* Reverse pass of the last checkpointed rollout.  Seeds dL/dx_T, dL/dv_T dev [B][3][N] (NULL = 0).  Outputs
  * (dev, each may be NULL, WRITTEN not accumulated): g_actions [H][B][G][6], g_x0, g_v0 [B][3][N],
@@ -151,6 +156,17 @@ dlo_status dlo_check_numerics(dlo_sim* sim, int32_t* n_bad);
  * is driven through the *_host calls additionally holds their device staging: 4 + 4 arrays [B][3][N], one [B][2][N],
  * one [B][5] and two [H][B][G][6] (actions, action gradients). */
 size_t dlo_scratch_bytes(const dlo_config* cfg, int32_t horizon, int32_t checkpoint_stride);
+
+/* Measurement.  dlo_set_kernel_timing(on != 0) makes the handle bracket every launch of its three big kernels with a
+ * CUDA event pair on the launching stream (and clears what was recorded before); dlo_get_kernel_timing synchronises and
+ * returns, for kernel_class 0 = forward segment kernel, 1 = the same with tape records (replay), 2 = segment adjoint
+ * kernel: the launches recorded, the sum of their durations and the env-steps they processed (each pointer host, may be
+ * NULL).  dlo_measure_fp32_peak runs an FFMA-chain microbenchmark (8 independent chains per thread, 2048 threads per SM,
+ * ~70 ms, best of 3) on the current device and returns the fp32 rate in TFLOP/s: the denominator of the ALU roofline
+ * (SURVEY.md section 8(d)); elapsed_ms, n_sm host, may be NULL. */
+dlo_status dlo_set_kernel_timing(dlo_sim* sim, int32_t on);
+dlo_status dlo_get_kernel_timing(dlo_sim* sim, int32_t kernel_class, int32_t* n_launches, double* total_ms, int64_t* env_steps);
+dlo_status dlo_measure_fp32_peak(void* cuda_stream, double* tflops, double* elapsed_ms, int32_t* n_sm);
 
 /* Number of kernel launches issued on this handle since create (bench.py's gpu_launches). */
 int64_t dlo_launch_count(const dlo_sim* sim);

@@ -29,6 +29,7 @@ struct EnvD {
   State<double> s0, cur;                 // state after A0 / current state
   std::vector<State<double>> ckpt;       // checkpoint g = state after g*stride steps
   std::vector<State<double>> rec;        // optional per-step record (rec[t] = state after t steps)
+  double margin[MG_COUNT];               // diagnostics: closest approach to each branch threshold during the last rollout
 };
 
 struct oracle_sim {
@@ -217,6 +218,8 @@ int32_t oracle_rollout_forward(oracle_sim* h, int32_t horizon, int32_t stride, i
     EnvD& e = h->env[b];
     Work<double> w;
     e.cur = e.s0; e.ckpt.clear(); e.rec.clear();
+    for (int k = 0; k < MG_COUNT; ++k) e.margin[k] = 1e300;
+    margin_sink() = e.margin;              // diagnostics only (rod_step.hpp, note_margin)
     if (stride > 0) e.ckpt.push_back(e.cur);
     if (record) e.rec.push_back(e.cur);
     static const double none[1] = {0.0};
@@ -227,8 +230,17 @@ int32_t oracle_rollout_forward(oracle_sim* h, int32_t horizon, int32_t stride, i
       if (stride > 0 && (t + 1) % stride == 0) e.ckpt.push_back(e.cur);
       if (record) e.rec.push_back(e.cur);
     }
+    margin_sink() = nullptr;
   }
   return 0;
+}
+
+// diagnostics: per env, the smallest relative distance to each branch threshold during the last oracle_rollout_forward
+// (classes MG_* of rod_step.hpp; 1e300 = the branch was never evaluated)
+int32_t oracle_num_margins(void) { return MG_COUNT; }
+void oracle_get_margins(oracle_sim* h, double* out /* [B][MG_COUNT] */) {
+  for (int b = 0; b < h->B; ++b)
+    for (int k = 0; k < MG_COUNT; ++k) out[(size_t)b * MG_COUNT + k] = h->env[b].margin[k];
 }
 
 static void pack_state(const Config& c, const State<double>& s, double* x, double* v, double* d1, double* kb) {

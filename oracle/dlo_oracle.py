@@ -32,7 +32,7 @@ def lib():
         _lib.oracle_op_bend_energy.restype = _F
         _lib.oracle_op_stretch_energy.restype = _F
         for name in ("oracle_rollout_forward", "oracle_backward", "oracle_get_record", "oracle_num_threads",
-                     "oracle_op_self_contact", "oracle_op_sdf"):
+                     "oracle_op_self_contact", "oracle_op_sdf", "oracle_num_margins"):
             getattr(_lib, name).restype = C.c_int32
     return _lib
 
@@ -45,6 +45,7 @@ def _ptr(a):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
 
 
+MARGIN_NAMES = ("approach", "stick", "f_kink", "f_threshold", "yield", "contact", "friction")   # MG_* of rod_step.hpp
 MATERIAL_KEYS = ("mass_per_vertex", "rest_edge_len", "stretch", "bend_stiffness", "damping", "yield_curv",
                  "creep_rate", "mu_rigid", "mu_self")
 
@@ -142,6 +143,16 @@ class OracleSim:
         if rc != 0:
             raise IndexError(t)
         return {"x": x, "v": v, "d1": d1, "kappa_bar": kb}
+
+    def margins(self):
+        """diagnostics: per env, the smallest relative distance to each branch threshold of the step during the last
+        rollout, as a dict of arrays [B] keyed by MARGIN_NAMES (inf = the branch was never evaluated)"""
+        L = lib()
+        n = int(L.oracle_num_margins())
+        out = np.zeros((self.B, n))
+        L.oracle_get_margins(self.h, _ptr(out))
+        out[out > 1e299] = np.inf
+        return {name: out[:, i] for i, name in enumerate(MARGIN_NAMES[:n])}
 
     def backward(self, dL_dxT=None, dL_dvT=None):
         B, N, G, H = self.B, self.N, self.G, self.H_done

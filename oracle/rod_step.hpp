@@ -236,6 +236,22 @@ void stretch_force(const Config& c, const std::vector<Vec3<T>>& x, const T& ks, 
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// DIAGNOSTICS ONLY (no arithmetic of the step depends on them): how close the trajectory comes to each branch of the
+// piecewise-smooth step, as the smallest relative distance to the threshold seen since the recorder was armed.  The
+// gradient of the step jumps where a branch flips (reading B-22: branches frozen at their forward outcome), so a test
+// that compares gradients needs to know when a trajectory runs along such a threshold.
+enum { MG_APPROACH = 0 /* |u_n| / |u| at the test u_n < 0 of a vertex inside the influence distance (L103) */,
+       MG_STICK /* |k| at the Coulomb stick / slide switch k > 0 of the soft coupling */,
+       MG_FKINK /* d / eps_s >= 0 on the saturated side of the kink of f = min(exp(d / eps_s), 1) */,
+       MG_FTHRESH /* |f - f_thresh| / f_thresh at the influence threshold (a jump of the VALUE, L103 "if f > 0.1") */,
+       MG_YIELD /* | |kappa_el| - Y | / Y at the Eq.11 yield test */,
+       MG_CONTACT /* |d| / (r_a + r_b) at the Eq.13 penetration test d > 0 of a candidate pair */,
+       MG_FRICTION /* |mu_s D_p / h - |v_t|| / |v_t| at the clamp of the self-contact friction (L410) */,
+       MG_COUNT };
+inline double*& margin_sink() { static thread_local double* p = nullptr; return p; }
+inline void note_margin(int cls, double rel) { double* m = margin_sink(); if (m && rel == rel && rel < m[cls]) m[cls] = rel; }
+
+// ---------------------------------------------------------------------------------------------------------
 // Eq.10 with XPBD compliance (reading B-8): one edge, in place on the correction accumulators.
 // e = current edge vector (x^p_{j+1}-x^p_j)+(dx_{j+1}-dx_j); atil = c/h^2 (0 => Eq.10 verbatim).
 template <class T>
@@ -273,6 +289,7 @@ inline bool self_contact_correction(const Vec3<T> x[4], const double w[4], doubl
   Vec3<T> dv = ca - cb;
   T delta = norm(dv);
   d = rsum - delta;
+  note_margin(MG_CONTACT, std::fabs(val(d)) / rsum);
   if (!(d > 0.0) || !(delta > 1e-12)) return false;
   n = (T(1.0) / delta) * dv;
   W = w[0] * (1.0 - t) * (1.0 - t) + w[1] * t * t + w[2] * (1.0 - u) * (1.0 - u) + w[3] * u * u;
@@ -289,6 +306,7 @@ template <class T>
 inline void plasticity_update(const T& k1, const T& k2, T& k1b, T& k2b, const T& Y, const T& r_c) {
   T e1 = k1 - k1b, e2 = k2 - k2b;
   T n = sqrt(e1 * e1 + e2 * e2);
+  note_margin(MG_YIELD, std::fabs(val(n) - val(Y)) / val(Y));
   if (n > Y) {
     T s = r_c * (n - Y) / n;
     k1b += s * e1;
@@ -372,17 +390,21 @@ template <class T>
 inline void rigid_response(Vec3<T>& v, const Vec3<T>& vb, const Vec3<T>& n, const T& d, double eps_s,
                            double f_thresh, double e_rest, double mu) {
   T f = exp(d / eps_s);
+  note_margin(MG_FTHRESH, std::fabs(val(f) - f_thresh) / f_thresh);
   if (f > 1.0) f = T(1.0);
   if (!(f > f_thresh)) return;
   Vec3<T> u = v - vb;
   T un = dot(u, n);
+  note_margin(MG_APPROACH, std::fabs(val(un)) / (std::sqrt(val(dot(u, u))) + 1e-300));
   if (!(un < 0.0)) return;
+  if (val(d) >= 0.0) note_margin(MG_FKINK, val(d) / eps_s);   // saturated side only: from below the response is smooth up to the kink
   Vec3<T> ut = u - un * n;
   T J = (1.0 + e_rest) * (-un);
   T utn = norm(ut);
   Vec3<T> utp = zero3<T>();
   if (utn > 1e-12) {
     T k = 1.0 - mu * J / utn;
+    if (mu > 0.0) note_margin(MG_STICK, std::fabs(val(k)));
     if (k > 0.0) utp = k * ut;
   }
   Vec3<T> up = (-e_rest * un) * n + utp;
@@ -533,6 +555,7 @@ void substep(const Config& c, const Scene& sc, const Params<T>& pm, State<T>& st
       T vtn = norm(vt);
       if (!(vtn > 1e-12)) continue;
       T cap = sc.mu_s * w.Dp[p] / h;
+      note_margin(MG_FRICTION, std::fabs(val(cap) - val(vtn)) / val(vtn));
       T mag = (cap < vtn) ? cap : vtn;
       Vec3<T> D = (-(mag / vtn)) * vt;
       w.acc[iv[0]] = w.acc[iv[0]] + (ws[0] * (1.0 - t) / W) * D;

@@ -12,8 +12,10 @@ from . import build as _build
 
 _F = C.c_float
 STATUS_CALLS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_primitives", "dlo_set_grippers", "dlo_set_state",
-                "dlo_restore_state", "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_backward",
-                "dlo_get_state_adjoint", "dlo_rollout_forward_host", "dlo_backward_host", "dlo_check_numerics")
+                "dlo_restore_state", "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_get_position_residual",
+                "dlo_backward",
+                "dlo_get_state_adjoint", "dlo_rollout_forward_host", "dlo_backward_host", "dlo_check_numerics",
+                "dlo_set_kernel_timing", "dlo_get_kernel_timing", "dlo_measure_fp32_peak")
 EXPORTS = STATUS_CALLS + ("dlo_scratch_bytes", "dlo_launch_count", "dlo_last_error", "dlo_version")
 MATERIAL_KEYS = ("mass_per_vertex", "rest_edge_len", "stretch", "bend_stiffness", "damping", "yield_curv",
                  "creep_rate", "mu_rigid", "mu_self")
@@ -120,8 +122,12 @@ def dlo_set_state(h, x0, v0, kappa_bar0=None):
     _chk(lib().dlo_set_state(h, _p(x0), _p(v0), _p(kappa_bar0)))
 
 
-def dlo_restore_state(h, x, v, d1, kappa_bar, step_index):
-    _chk(lib().dlo_restore_state(h, _p(x), _p(v), _p(d1), _p(kappa_bar), C.c_int32(step_index)))
+def dlo_restore_state(h, x, x_lo, v, d1, kappa_bar, step_index):
+    _chk(lib().dlo_restore_state(h, _p(x), _p(x_lo), _p(v), _p(d1), _p(kappa_bar), C.c_int32(step_index)))
+
+
+def dlo_get_position_residual(h, x_lo):
+    _chk(lib().dlo_get_position_residual(h, _p(x_lo)))
 
 
 def dlo_get_state_adjoint(h, g_x=None, g_v=None, g_d1=None, g_kappa_bar=None):
@@ -159,6 +165,24 @@ def dlo_check_numerics(h):
     if st not in (0, -6):
         _chk(st)
     return int(n.value)
+
+
+def dlo_set_kernel_timing(h, on):
+    _chk(lib().dlo_set_kernel_timing(h, C.c_int32(1 if on else 0)))
+
+
+def dlo_get_kernel_timing(h, kernel_class):
+    """(launches, total ms, env-steps) of kernel class 0 forward / 1 replay / 2 adjoint since dlo_set_kernel_timing(on)"""
+    n, ms, units = C.c_int32(0), C.c_double(0.0), C.c_int64(0)
+    _chk(lib().dlo_get_kernel_timing(h, C.c_int32(kernel_class), C.byref(n), C.byref(ms), C.byref(units)))
+    return int(n.value), float(ms.value), int(units.value)
+
+
+def dlo_measure_fp32_peak(stream=0):
+    """(TFLOP/s, elapsed ms, SM count) of the FFMA-chain microbenchmark on the current device"""
+    tf, ms, n = C.c_double(0.0), C.c_double(0.0), C.c_int32(0)
+    _chk(lib().dlo_measure_fp32_peak(C.c_void_p(stream), C.byref(tf), C.byref(ms), C.byref(n)))
+    return float(tf.value), float(ms.value), int(n.value)
 
 
 def dlo_scratch_bytes(cfg: DloConfig, horizon, checkpoint_stride):
@@ -231,18 +255,29 @@ class DloSim:
         dlo_set_state(self.h, self.x0, self.v0, self.kb0)
 
     def restore(self, state, step_index):
-        """exact restore of a state dict (x, v, d1, kappa_bar: numpy or device tensors) as the start of the next rollout"""
-        t = {k: (state[k] if hasattr(state[k], "data_ptr") else self._up(state[k])) for k in ("x", "v", "d1", "kappa_bar")}
+        """exact restore of a state dict (x, v, d1, kappa_bar and optionally x_lo: numpy or device tensors) as the start
+        of the next rollout.  fp64 numpy positions without an x_lo are split into their nearest fp32 and the fp32 residual."""
+        t = {k: (state[k] if hasattr(state[k], "data_ptr") else self._up(state[k])) for k in ("v", "d1", "kappa_bar")}
+        x, xl = state["x"], state.get("x_lo")
+        if hasattr(x, "data_ptr"):
+            t["x"], t["x_lo"] = x, xl
+        else:
+            a = np.asarray(x, dtype=np.float64)
+            hi = a.astype(np.float32)
+            t["x"] = self._up(hi)
+            t["x_lo"] = self._up((a - hi.astype(np.float64)).astype(np.float32) if xl is None else xl)
         self._restored = t
-        dlo_restore_state(self.h, t["x"], t["v"], t["d1"], t["kappa_bar"], int(step_index))
+        dlo_restore_state(self.h, t["x"], t["x_lo"], t["v"], t["d1"], t["kappa_bar"], int(step_index))
 
     def state_device(self):
         """current state as fp32 device tensors (no host copy)"""
         torch = self.torch
         B, N = self.B, self.N
         out = {"x": torch.empty((B, 3, N), device=self.dev), "v": torch.empty((B, 3, N), device=self.dev),
-               "d1": torch.empty((B, 3, N), device=self.dev), "kappa_bar": torch.empty((B, 2, N), device=self.dev)}
+               "d1": torch.empty((B, 3, N), device=self.dev), "kappa_bar": torch.empty((B, 2, N), device=self.dev),
+               "x_lo": torch.empty((B, 3, N), device=self.dev)}
         dlo_get_state(self.h, out["x"], out["v"], out["d1"], out["kappa_bar"])
+        dlo_get_position_residual(self.h, out["x_lo"])
         return out
 
     def state_adjoint(self):
@@ -267,9 +302,12 @@ class DloSim:
         B, N = self.B, self.N
         x, v, d1 = (torch.empty((B, 3, N), device=self.dev) for _ in range(3))
         kb = torch.empty((B, 2, N), device=self.dev)
+        xl = torch.empty((B, 3, N), device=self.dev)
         dlo_get_state(self.h, x, v, d1, kb)
+        dlo_get_position_residual(self.h, xl)
         torch.cuda.synchronize(self.dev)
-        return {"x": x.double().cpu().numpy(), "v": v.double().cpu().numpy(), "d1": d1.double().cpu().numpy(),
+        # positions as the library carries them: x + x_lo, summed in fp64
+        return {"x": (x.double() + xl.double()).cpu().numpy(), "v": v.double().cpu().numpy(), "d1": d1.double().cpu().numpy(),
                 "kappa_bar": kb.double().cpu().numpy()}
 
     def backward(self, dL_dxT=None, dL_dvT=None):

@@ -62,6 +62,23 @@ struct dlo_sim {
   float *dx0 = nullptr, *dv0 = nullptr, *dkb = nullptr, *dact = nullptr, *dxT = nullptr, *dvT = nullptr;
   float *dsx = nullptr, *dsv = nullptr, *dga = nullptr, *dgx = nullptr, *dgv = nullptr, *dgm = nullptr;
   size_t hact_n = 0, dact_n = 0, dga_n = 0;
+  // optional per-kernel timing (dlo_set_kernel_timing): CUDA event pairs around every launch of the three big kernels,
+  // recorded on the stream the kernel is launched on; class 0 = k_forward, 1 = k_forward with tape (replay), 2 = k_adjoint
+  bool timing = false;
+  std::vector<cudaEvent_t> tev[3];   // start, stop, start, stop, ...
+  std::vector<int64_t> tunits[3];    // env-steps processed by each launch
+};
+
+struct LaunchTimer {   // brackets one launch with an event pair when timing is on
+  dlo_sim* s; int cls; cudaStream_t st; cudaEvent_t stop = nullptr;
+  LaunchTimer(dlo_sim* s_, int cls_, cudaStream_t st_, int64_t units) : s(s_), cls(cls_), st(st_) {
+    if (!s->timing) return;
+    cudaEvent_t a = nullptr;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&stop) != cudaSuccess) { if (a) cudaEventDestroy(a); stop = nullptr; cudaGetLastError(); return; }
+    cudaEventRecord(a, st);
+    s->tev[cls].push_back(a); s->tev[cls].push_back(stop); s->tunits[cls].push_back(units);
+  }
+  ~LaunchTimer() { if (stop) cudaEventRecord(stop, st); }
 };
 
 // every entry point: the handle's device must be the current one
@@ -275,6 +292,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
   for (void* p : dev) if (p) cudaFree(p);
   if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
   for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
+  for (auto& v : s->tev) for (cudaEvent_t e : v) cudaEventDestroy(e);
   void* stg[] = {s->dx0, s->dv0, s->dkb, s->dact, s->dxT, s->dvT, s->dsx, s->dsv, s->dga, s->dgx, s->dgv, s->dgm};
   for (void* p : stg) if (p) cudaFree(p);
   void* host[] = {s->hx0, s->hv0, s->hkb, s->hact, s->hxT, s->hvT};
@@ -344,14 +362,14 @@ dlo_status dlo_set_state(dlo_sim* s, const float* x0, const float* v0, const flo
   return DLO_OK;
 }
 
-dlo_status dlo_restore_state(dlo_sim* s, const float* x, const float* v, const float* d1, const float* kb, int32_t step_index) {
+dlo_status dlo_restore_state(dlo_sim* s, const float* x, const float* x_lo, const float* v, const float* d1, const float* kb, int32_t step_index) {
   ENTER(s);
   if (!x || !v || !d1 || !kb) return fail(DLO_ERR_INVALID_ARG, "NULL argument (x, v, d1 and kappa_bar are all required)");
   if (step_index < 0) return fail(DLO_ERR_INVALID_ARG, "step_index < 0");
   if (!s->have_q) return fail(DLO_ERR_BAD_STATE, "dlo_restore_state needs an earlier dlo_set_state on this scene (grasp-local coordinates are captured there)");
   const KParams& P = s->P;
   const size_t n = (size_t)P.B * s->blk;
-  k_put_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, x, v, d1, kb, s->state0);
+  k_put_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, x, v, d1, kb, x_lo, s->state0);
   s->launches += 1;
   CU(cudaGetLastError());
   CU(cudaMemcpyAsync(s->state, s->state0, n * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
@@ -374,7 +392,10 @@ template <int VPL, bool TAPE> static cudaError_t launch_forward_t(dlo_sim* s, co
   cudaError_t e = cudaFuncSetAttribute(k_forward<VPL, TAPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fwd > 48 * 1024 ? s->smem_fwd : 48 * 1024);
   if (e != cudaSuccess) return e;
   const int grid = (P.B + s->wpb_fwd - 1) / s->wpb_fwd;
-  k_forward<VPL, TAPE><<<grid, s->wpb_fwd * 32, s->smem_fwd, st>>>(P, t0, t1, stride);
+  {
+    LaunchTimer lt(s, TAPE ? 1 : 0, st, (int64_t)P.B * (t1 - t0));
+    k_forward<VPL, TAPE><<<grid, s->wpb_fwd * 32, s->smem_fwd, st>>>(P, t0, t1, stride);
+  }
   s->launches += 1;
   return cudaGetLastError();
 }
@@ -528,7 +549,19 @@ dlo_status dlo_get_state(dlo_sim* s, float* x, float* v, float* d1, float* kb) {
   if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "no state");
   const KParams& P = s->P;
   const size_t n = (size_t)P.B * STATE_ROWS * P.N;
-  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, s->state, x, v, d1, kb);
+  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, s->state, x, v, d1, kb, nullptr);
+  s->launches += 1;
+  CU(cudaGetLastError());
+  return DLO_OK;
+}
+
+dlo_status dlo_get_position_residual(dlo_sim* s, float* x_lo) {
+  ENTER(s);
+  if (!x_lo) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  if (!s->have_state) return fail(DLO_ERR_BAD_STATE, "no state");
+  const KParams& P = s->P;
+  const size_t n = (size_t)P.B * STATE_ROWS * P.N;
+  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(P.B, P.N, P.NS, s->state, nullptr, nullptr, nullptr, nullptr, x_lo);
   s->launches += 1;
   CU(cudaGetLastError());
   return DLO_OK;
@@ -549,3 +582,4 @@ dlo_status dlo_check_numerics(dlo_sim* s, int32_t* n_bad) {
 }  // extern "C"
 
 #include "dlo_api_backward.inl"
+#include "dlo_bench.inl"

@@ -4,7 +4,10 @@ template <int VPL> static cudaError_t launch_adjoint_t(dlo_sim* s, const KParams
   cudaError_t e = cudaFuncSetAttribute(k_adjoint<VPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_adj > 48 * 1024 ? s->smem_adj : 48 * 1024);
   if (e != cudaSuccess) return e;
   const int grid = (P.B + s->wpb_adj - 1) / s->wpb_adj;
-  k_adjoint<VPL><<<grid, s->wpb_adj * 32, s->smem_adj, s->stream>>>(P, t0, t1);
+  {
+    LaunchTimer lt(s, 2, s->stream, (int64_t)P.B * (t1 - t0));
+    k_adjoint<VPL><<<grid, s->wpb_adj * 32, s->smem_adj, s->stream>>>(P, t0, t1);
+  }
   s->launches += 1;
   return cudaGetLastError();
 }
@@ -109,7 +112,7 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   }
   if (g_x0 || g_v0) {
     const size_t n = (size_t)B * STATE_ROWS * s->P.N;
-    k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, s->adj, g_x0, g_v0, nullptr, nullptr);
+    k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(B, s->P.N, s->P.NS, s->adj, g_x0, g_v0, nullptr, nullptr, nullptr);
     s->launches += 1;
     CU(cudaGetLastError());
   }
@@ -122,7 +125,7 @@ dlo_status dlo_get_state_adjoint(dlo_sim* s, float* g_x, float* g_v, float* g_d1
   ENTER(s);
   if (!s->have_adj) return fail(DLO_ERR_BAD_STATE, "dlo_get_state_adjoint needs a completed dlo_backward");
   const size_t n = (size_t)s->P.B * STATE_ROWS * s->P.N;
-  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->P.B, s->P.N, s->P.NS, s->adj, g_x, g_v, g_d1, g_kb);
+  k_get_state<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->P.B, s->P.N, s->P.NS, s->adj, g_x, g_v, g_d1, g_kb, nullptr);
   s->launches += 1;
   CU(cudaGetLastError());
   return DLO_OK;

@@ -32,7 +32,7 @@ template <int VPL> __device__ __forceinline__ void store_adj(float* __restrict__
 }
 
 enum { GM_STRETCH = 0, GM_ALPHA = 1, GM_GAMMA = 2, GM_SIGY = 3, GM_RC = 4 };
-struct GradAcc { float gm[5], apbar[6], acbar[6]; };
+struct GradAcc { double gm[5]; float apbar[6], acbar[6]; };   // material adjoints: sums of cancelling terms over all substeps, kept in double
 
 // add `val` to the array element at the lane's last valid slot
 template <int VPL> __device__ __forceinline__ void add_at_last(f3 a[VPL], int ks, const f3& val) {
@@ -85,7 +85,7 @@ __device__ __forceinline__ bool body_eval(const KParams& P, const WarpSmem& sm, 
   const float* Bp = o + (fk ? POSE_FB1 : POSE_FB0);
   const float Pc[7] = {A[0], A[1], A[2], Bp[0], Bp[1], Bp[2], o[POSE_RF]};
   if (!sdf_eval<float>(1, Pc, y, phi, n)) return false;
-  vb = body_point_velocity<float>(read_pose(o, 0), read_pose(o, 1), y, P.inv_h);
+  vb = finger_body_velocity(o, y, P.inv_h);   // the forward's expression: same bits, same branches
   return true;
 }
 

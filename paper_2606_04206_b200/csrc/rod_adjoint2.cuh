@@ -26,7 +26,7 @@ __device__ __forceinline__ void edge_reverse(const f3& epred, float lam, float w
 // The same with the loop invariants precomputed (idn = 1 / (wk + wn + atil), 0 for a slot that is not projected) and no
 // branch: an idle slot has lam = 0 on the tape and idn = 0, so every update below adds a zero.
 __device__ __forceinline__ void edge_reverse_pre(const f3& epred, float lam, float wk, float wn, float idn, float atil, f3& dxk, f3& dxn, float& S,
-                                                 f3& gk, f3& gn, float& Sb, float& atilbar, f3& epb) {
+                                                 f3& gk, f3& gn, float& Sb, double& atilbar, f3& epb) {
   const f3 ep = epred + (dxn - dxk);                // = (L - lam (wk+wn)) t
   const float ep2 = fmaxf(dot(ep, ep), 1.0e-30f);   // (padding slots have ep = 0: keep t finite)
   const float iLp = rsqrt_(ep2);
@@ -39,7 +39,7 @@ __device__ __forceinline__ void edge_reverse_pre(const f3& epred, float lam, flo
   // project_edge_adj (rod_adj.cuh) with the division by (wk + wn + atil) replaced by the stored reciprocal
   const f3 g = wk * gk - wn * gn;
   const float numbar = (dot(g, t) + Sb) * idn;
-  atilbar -= numbar * Spost;
+  atilbar -= (double)numbar * (double)Spost;   // thousands of terms of either sign per substep: summed in double
   Sb -= atil * numbar;
   const f3 tbar = lam * g;
   const f3 eb = numbar * t + (1.0f / L) * (tbar - dot(tbar, t) * t);
@@ -55,6 +55,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
                                                 const float ap[6], const float ac[6], int sub, const float* __restrict__ s0blk,
                                                 const float* __restrict__ s1blk, LaneAdj<VPL>& A, GradAcc& G, float* acc_tape, int contact_flag, int side_slot) {
   const float h = P.h, inv_h = P.inv_h;
+  float gm_rc = 0.0f, gm_sigy = 0.0f, gm_gamma = 0.0f;   // this substep's share of the material adjoints (a few terms per lane);
+                                                         // the sums over substeps run in double (G.gm): they cancel heavily
   // ---- forward recompute with recording.  The start state is read from the tape twice (here and again for the
   // reverse of A2) rather than held in ~70 registers across the projection loop, the hottest part of the kernel.
   LaneState<VPL> s0;
@@ -75,27 +77,26 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     substep<VPL, 1>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, acc_tape, cc, const_cast<float*>(s0blk) + (size_t)TAPE_LAM * P.NS);
   } else {
     // common case: everything the reverse needs is on the tape record written by the replay
-    load_rows3<VPL>(s0blk + (size_t)TAPE_XP * P.NS, tp.base, P.NS, R.xp);
     load_rows3<VPL>(s0blk + (size_t)TAPE_DX * P.NS, tp.base, P.NS, R.dx);
-    load_rows3<VPL>(s0blk + (size_t)TAPE_V3 * P.NS, tp.base, P.NS, R.v3);
+    load_rows3<VPL>(s0blk + (size_t)TAPE_V1 * P.NS, tp.base, P.NS, R.v1);
     load_row<VPL>(s0blk + (size_t)TAPE_S * P.NS, tp.base, P.NS, R.S);
     float am[VPL];
     load_row<VPL>(s0blk + (size_t)TAPE_ACT * P.NS, tp.base, P.NS, am);
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
       R.active[k] = __float_as_uint(am[k]);
-      R.v1[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v3[k], -inv_h, R.dx[k]) : R.v3[k];   // v^3 = v^1 + dx/h without friction
+      R.v3[k] = (c.kin[k] == KIN_FREE) ? axpy(R.v1[k], inv_h, R.dx[k]) : R.v1[k];   // v^3 = v^1 + dx/h without friction (the forward's expression)
       R.t_old[k] = ec0.t[k];
     }
     R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u;
     if (contact_flag == 2) {
-      // self-contact data of the substep from its side record: candidate list, depth sums, v^1 (v^3 includes friction here);
+      // self-contact data of the substep from its side record: candidate list, depth sums, v^3 (which includes friction here);
       // the summed corrections of the Jacobi passes are read from the record in the reverse loop
       const float* sr = P.side + (size_t)side_slot * P.side_floats;
       R.ncand = reinterpret_cast<const int*>(sr)[0];
       R.jac_mask = reinterpret_cast<const unsigned*>(sr)[1];
       R.any_pen = 1;
-      load_rows3<VPL>(sr + side_off_v1(), tp.base, P.NS, R.v1);
+      load_rows3<VPL>(sr + side_off_v3(), tp.base, P.NS, R.v3);
       const unsigned* cs = reinterpret_cast<const unsigned*>(sr + side_off_cand(P));
       unsigned* cd = reinterpret_cast<unsigned*>(sm.cand);
       for (int p = tp.lane; p < (R.ncand + 1) / 2; p += 32) cd[p] = cs[p];
@@ -107,12 +108,15 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     }
     // state at the end of the substep = start state of the next record (positions and directors are all that is used)
     load_rows3<VPL>(s1blk + (size_t)ROW_X * P.NS, tp.base, P.NS, s.x);
+    load_rows3<VPL>(s1blk + (size_t)ROW_XL * P.NS, tp.base, P.NS, s.xl);
     load_rows3<VPL>(s1blk + (size_t)ROW_D1 * P.NS, tp.base, P.NS, s.d1);
     edge_refresh<VPL>(tp, s, ec);
     edge_prev_refresh<VPL>(tp, s, ec);
     substep_idle_syncs(P, sm);
   }
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose);   // keep this substep's poses for the reverse
+#pragma unroll
+  for (int k = 0; k < VPL; ++k) R.xp[k] = axpy(s0.x[k], h, R.v1[k]);   // x^p by the forward's own expression: same bits
 
   f3 tbar_old[VPL], tbar_new[VPL];
 #pragma unroll
@@ -131,8 +135,8 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         float k1, k2;
         material_curvature<float>(ta, ec.t[k], da, s.d1[k], k1, k2);
         float k1bar = 0.f, k2bar = 0.f, Ybar = 0.f;
-        plasticity_adj<float>(k1, k2, s0.kb1[k], s0.kb2[k], Y, c.rc, A.kb1[k], A.kb2[k], k1bar, k2bar, Ybar, G.gm[GM_RC]);
-        G.gm[GM_SIGY] += Ybar * c.l0;
+        plasticity_adj<float>(k1, k2, s0.kb1[k], s0.kb2[k], Y, c.rc, A.kb1[k], A.kb2[k], k1bar, k2bar, Ybar, gm_rc);
+        gm_sigy += Ybar * c.l0;
         f3 tab = zero3<float>(), tbb = zero3<float>(), dab = zero3<float>(), dbb = zero3<float>();
         material_curvature_adj<float>(ta, ec.t[k], da, s.d1[k], k1bar, k2bar, tab, tbb, dab, dbb);
         tbar_new[k] += tbb;
@@ -234,12 +238,17 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 
   phase_sync(sm);
   // ---- reverse A5: iterations backwards; each Eq.10 update is undone from its stored multiplier
-  const f3 xpr = shfl3(R.xp[0], tp.nl);
-  f3 epred[VPL];
+  f3 epred[VPL];   // the forward's predicted edge vectors, by the forward's expression (positions re-read: they are not held across the reverse of A9..A6)
+  {
+    LaneState<VPL> sx;
+    load_rows3<VPL>(s0blk + (size_t)ROW_X * P.NS, tp.base, P.NS, sx.x);
+    load_rows3<VPL>(s0blk + (size_t)ROW_XL * P.NS, tp.base, P.NS, sx.xl);
+    const f3 xr = shfl3(sx.x[0], tp.nl), xlr = shfl3(sx.xl[0], tp.nl), v1r = shfl3(R.v1[0], tp.nl);
 #pragma unroll
-  for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
+    for (int k = 0; k < VPL; ++k) epred[k] = axpy(edge_vec<VPL>(sx, xr, xlr, k, tp.ks), h, next_of<VPL>(R.v1, v1r, k, tp.ks) - R.v1[k]);
+  }
   const float atil = c.stretch * inv_h * inv_h;
-  float atilbar = 0.0f;
+  double atilbar = 0.0;   // adjoint of the compliance term alpha~ = c / h^2: a sum of nearly cancelling terms
   float idn[VPL], wfar[VPL];   // as in substep(): far-vertex inverse mass, 1 / (w_j + w_j+1 + atil) or 0 for an idle slot
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
@@ -283,9 +292,9 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
           // the compiler index them by ks, which puts them in local memory for the whole kernel
           const bool on = (k == tp.ks) && (tp.base + k == P.E - 1) && (c.w[k] + c.wr > 0.0f);
           f3 dxk = R.dx[k], dxn = dxr, gk = dxb[k], gn = gr, eb = epb[k];
-          float Sk = R.S[k], sb = Sb[k], ab = atilbar;
+          float Sk = R.S[k], sb = Sb[k], ab = 0.0f;
           if (on) edge_reverse(epred[k], lamv[k], c.w[k], c.wr, atil, dxk, dxn, Sk, gk, gn, sb, ab, eb);
-          R.dx[k] = dxk; dxr = dxn; R.S[k] = Sk; dxb[k] = gk; gr = gn; Sb[k] = sb; atilbar = ab; epb[k] = eb;
+          R.dx[k] = dxk; dxr = dxn; R.S[k] = Sk; dxb[k] = gk; gr = gn; Sb[k] = sb; atilbar += (double)ab; epb[k] = eb;
         }
         R.dx[0] += shfl3(dxr - dxr0, tp.pl);
         dxb[0] += shfl3(gr - gr0, tp.pl);
@@ -314,7 +323,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         edge_reverse_pre(epred[k], idn[k] != 0.0f ? lamv[k] : 0.0f, c.w[k], wfar[k], idn[k], atil, R.dx[k], R.dx[k + 1], R.S[k], dxb[k], dxb[k + 1], Sb[k], atilbar, epb[k]);
     }
   }
-  G.gm[GM_STRETCH] += (P.stretch_mode == 1) ? atilbar * inv_h * inv_h : 0.0f;
+  G.gm[GM_STRETCH] += (P.stretch_mode == 1) ? atilbar * (double)inv_h * (double)inv_h : 0.0;
   {   // predicted edge vectors -> predicted positions
     f3 send = zero3<float>();
 #pragma unroll
@@ -337,7 +346,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     if (c.kin[k] == KIN_FREE) {
       A.v[k] = idamp * v1bar[k];
       fbar[k] = (hm * idamp) * v1bar[k];
-      G.gm[GM_GAMMA] -= h * idamp * dot(v1bar[k], R.v1[k]);
+      gm_gamma -= h * idamp * dot(v1bar[k], R.v1[k]);
     } else if (c.kin[k] >= KIN_GRASP0) {
       const f3 tb = inv_h * v1bar[k];
       ga.add(P, sm, c.kin[k], tb);
@@ -377,7 +386,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         else { tb2[k > 0 ? k - 1 : 0] += tab; A.d1[k > 0 ? k - 1 : 0] += dab; ib2[k > 0 ? k - 1 : 0] += iab; }
       }
     }
-    G.gm[GM_ALPHA] += sbar / c.l0;
+    G.gm[GM_ALPHA] += (double)(sbar / c.l0);
     add_at_last<VPL>(tb2, tp.ks, shfl3(ptb, tp.nl));
     add_at_last<VPL>(A.d1, tp.ks, shfl3(pdb, tp.nl));
     add_at_last<VPL>(ib2, tp.ks, shfl(piLb, tp.nl));
@@ -387,7 +396,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
         if (tp.evalid[k]) {
           const f3 Fb = fbar[k] - next_of<VPL>(fbar, fb_next, k, tp.ks);
           const float L = 1.0f / eb0.iL[k], eps = L / c.l0 - 1.0f, Ft = dot(Fb, eb0.t[k]);
-          G.gm[GM_STRETCH] += eps * Ft;
+          G.gm[GM_STRETCH] += (double)(eps * Ft);
           tb2[k] += (c.stretch * eps) * Fb;
           ib2[k] -= (c.stretch * Ft / c.l0) * L * L;
         }
@@ -400,6 +409,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.x[0] += shfl3(send, tp.pl);
   }
 
+  G.gm[GM_RC] += (double)gm_rc; G.gm[GM_SIGY] += (double)gm_sigy; G.gm[GM_GAMMA] += (double)gm_gamma;
   phase_sync(sm);
   // ---- reverse A1: pose adjoints -> action adjoints (lane g owns gripper g)
   if (P.G > 0) {
@@ -439,7 +449,7 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
   load_adj<VPL>(P.adj + (size_t)env * blk, tp.base, P.NS, A);
   GradAcc G;
 #pragma unroll
-  for (int k = 0; k < 5; ++k) G.gm[k] = 0.0f;
+  for (int k = 0; k < 5; ++k) G.gm[k] = 0.0;
   float ap[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, ac[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
   float* acc_tape = P.acc_tape ? P.acc_tape + (size_t)env * P.N_C * 3 * sm.NP : nullptr;
   for (int t = t1 - 1; t >= t0; --t) {
@@ -450,6 +460,10 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
       const size_t rec = (size_t)tape_rows(P.N_C) * P.NS, idx = (size_t)(t - t0) * P.n_sub + sub;
       const float* s0blk = P.tape + (idx * P.B + env) * rec;
       const float* s1blk = P.tape + ((idx + 1) * P.B + env) * rec;
+      // the record of the substep reversed NEXT goes to L2 now (one bulk prefetch, no registers, no shared memory): with two
+      // warps per scheduler there is nothing to hide a DRAM round trip behind when its rows are loaded
+      if (idx > 0 && tp.lane == 0)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(P.tape + ((idx - 1) * P.B + env) * rec), "r"((unsigned)(rec * sizeof(float))) : "memory");
       const int cflag = P.tape_flag ? (int)P.tape_flag[idx * P.B + env] : 1;
       const int slot = (cflag == 2) ? P.tape_slot[idx * P.B + env] : -1;
       substep_reverse<VPL>(P, tp, c, sm, env, ap, ac, sub, s0blk, s1blk, A, G, acc_tape, cflag, slot);
@@ -468,8 +482,10 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
   store_adj<VPL>(P.adj + (size_t)env * blk, tp.base, P.NS, A);
 #pragma unroll
   for (int k = 0; k < 5; ++k) {
-    const float tot = warp_sum(G.gm[k]);
-    if (tp.lane == 0) P.gmat[(size_t)env * 5 + k] += tot;
+    double v = G.gm[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(DLO_FULL, v, o);
+    if (tp.lane == 0) P.gmat[(size_t)env * 5 + k] += (float)v;
   }
 }
 

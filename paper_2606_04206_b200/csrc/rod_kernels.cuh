@@ -113,7 +113,7 @@ __global__ void k_pack_material(int B, MatArgs m, float* out) {
 }
 
 // internal state block -> user arrays (any may be null)
-__global__ void k_get_state(int B, int N, int NS, const float* state, float* x, float* v, float* d1, float* kb) {
+__global__ void k_get_state(int B, int N, int NS, const float* state, float* x, float* v, float* d1, float* kb, float* xl) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)B * STATE_ROWS * N) return;
   const int i = (int)(idx % N), q = (int)((idx / N) % STATE_ROWS), env = (int)(idx / ((size_t)N * STATE_ROWS));
@@ -121,11 +121,12 @@ __global__ void k_get_state(int B, int N, int NS, const float* state, float* x, 
   if (q < 3) { if (x) x[((size_t)env * 3 + q) * N + i] = val; }
   else if (q < 6) { if (v) v[((size_t)env * 3 + q - 3) * N + i] = val; }
   else if (q < 9) { if (d1) d1[((size_t)env * 3 + q - 6) * N + i] = val; }
-  else if (kb) kb[((size_t)env * 2 + q - 9) * N + i] = val;
+  else if (q < 11) { if (kb) kb[((size_t)env * 2 + q - 9) * N + i] = val; }
+  else if (xl) xl[((size_t)env * 3 + q - 11) * N + i] = val;
 }
 
 // user arrays -> internal state block (exact restore: the inverse of k_get_state; padding columns zeroed)
-__global__ void k_put_state(int B, int N, int NS, const float* x, const float* v, const float* d1, const float* kb, float* state) {
+__global__ void k_put_state(int B, int N, int NS, const float* x, const float* v, const float* d1, const float* kb, const float* xl, float* state) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (size_t)B * STATE_ROWS * NS) return;
   const int i = (int)(idx % NS), q = (int)((idx / NS) % STATE_ROWS), env = (int)(idx / ((size_t)NS * STATE_ROWS));
@@ -134,7 +135,8 @@ __global__ void k_put_state(int B, int N, int NS, const float* x, const float* v
     if (q < 3) val = x[((size_t)env * 3 + q) * N + i];
     else if (q < 6) val = v[((size_t)env * 3 + q - 3) * N + i];
     else if (q < 9) val = d1[((size_t)env * 3 + q - 6) * N + i];
-    else val = kb[((size_t)env * 2 + q - 9) * N + i];
+    else if (q < 11) val = kb[((size_t)env * 2 + q - 9) * N + i];
+    else val = xl ? xl[((size_t)env * 3 + q - 11) * N + i] : 0.0f;
   }
   state[idx] = val;
 }
@@ -245,9 +247,8 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
         float* tb = P.tape + (idx * P.B + env) * rec;
         store_state<VPL>(tb, tp.base, P.NS, s);
         substep<VPL, 2>(P, tp, c, sm, env, ap, ac, sub, s, ec, R, nullptr, cc, tb + (size_t)TAPE_LAM * P.NS);
-        // (the x^p rows are stored inside substep, as soon as they exist: fewer registers live across its projection loop)
         store_rows3<VPL>(tb + (size_t)TAPE_DX * P.NS, tp.base, P.NS, R.dx);
-        store_rows3<VPL>(tb + (size_t)TAPE_V3 * P.NS, tp.base, P.NS, R.v3);
+        store_rows3<VPL>(tb + (size_t)TAPE_V1 * P.NS, tp.base, P.NS, R.v1);
         store_row<VPL>(tb + (size_t)TAPE_S * P.NS, tp.base, P.NS, R.S);
         float am[VPL];
 #pragma unroll
@@ -257,7 +258,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
         if (R.any_pen && R.side_slot >= 0) {   // what the reverse pass needs of this substep's self-contact, so that it need not recompute it
           float* sr = P.side + (size_t)R.side_slot * P.side_floats;
           if (tp.lane == 0) { reinterpret_cast<int*>(sr)[0] = R.ncand; reinterpret_cast<unsigned*>(sr)[1] = R.jac_mask; P.tape_slot[idx * P.B + env] = R.side_slot; }
-          store_rows3<VPL>(sr + side_off_v1(), tp.base, P.NS, R.v1);
+          store_rows3<VPL>(sr + side_off_v3(), tp.base, P.NS, R.v3);
           const unsigned* cs = reinterpret_cast<const unsigned*>(sm.cand);
           unsigned* cd = reinterpret_cast<unsigned*>(sr + side_off_cand(P));
           for (int p = tp.lane; p < (R.ncand + 1) / 2; p += 32) cd[p] = cs[p];

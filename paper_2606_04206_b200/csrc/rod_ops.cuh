@@ -61,6 +61,10 @@ DLO_HD void sincos_(float a, float* s, float* c) {
 #endif
 }
 DLO_HD void sincos_(double a, double* s, double* c) { *s = sin(a); *c = cos(a); }
+// explicit fused multiply-add: used where the SAME value must come out of every kernel the expression is inlined into
+// (forward, replay, reverse pass): an `a * b + c` left to the compiler may be contracted differently in each of them
+DLO_HD float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+DLO_HD double fma_(double a, double b, double c) { return fma(a, b, c); }
 template <class T> DLO_HD T clamp01(T s) { return s < T(0) ? T(0) : (s > T(1) ? T(1) : s); }
 
 // 3x3 rotation, row-major
@@ -76,17 +80,18 @@ template <class T> DLO_HD V3<T> mulT(const M3<T>& R, const V3<T>& a) {
 
 // Rodrigues coefficients: R = I + A [rho]x + B [rho]x^2, series for |rho|^2 < 1e-8 (R-20)
 template <class T> DLO_HD void rodrigues_coeff(T th2, T& A, T& B) {
-  if (th2 < T(1e-8)) { A = T(1) - th2 / T(6); B = T(0.5) - th2 / T(24); }
+  if (th2 < T(1e-8)) { A = fma_(th2, T(-1.0 / 6.0), T(1)); B = fma_(th2, T(-1.0 / 24.0), T(0.5)); }
   else { T th = sqrt_(th2), s, c; sincos_(th, &s, &c); A = s / th; B = (T(1) - c) / th2; }
 }
 template <class T> DLO_HD M3<T> rodrigues(const V3<T>& rho) {
-  T th2 = dot(rho, rho), A, B;
-  rodrigues_coeff(th2, A, B);
   const T kx = rho.x, ky = rho.y, kz = rho.z;
+  T th2 = fma_(kz, kz, fma_(ky, ky, kx * kx)), A, B;
+  rodrigues_coeff(th2, A, B);
+  const T Bx = B * kx, By = B * ky, Ax = A * kx, Ay = A * ky, Az = A * kz;   // every sum of products below is an explicit fma
   M3<T> R;
-  R.m[0] = T(1) + B * (kx * kx - th2); R.m[1] = -A * kz + B * kx * ky;      R.m[2] = A * ky + B * kx * kz;
-  R.m[3] = A * kz + B * kx * ky;      R.m[4] = T(1) + B * (ky * ky - th2); R.m[5] = -A * kx + B * ky * kz;
-  R.m[6] = -A * ky + B * kx * kz;     R.m[7] = A * kx + B * ky * kz;       R.m[8] = T(1) + B * (kz * kz - th2);
+  R.m[0] = fma_(B, fma_(kx, kx, -th2), T(1)); R.m[1] = fma_(Bx, ky, -Az);                R.m[2] = fma_(Bx, kz, Ay);
+  R.m[3] = fma_(Bx, ky, Az);                 R.m[4] = fma_(B, fma_(ky, ky, -th2), T(1)); R.m[5] = fma_(By, kz, -Ax);
+  R.m[6] = fma_(Bx, kz, -Ay);                R.m[7] = fma_(By, kz, Ax);                 R.m[8] = fma_(B, fma_(kz, kz, -th2), T(1));
   return R;
 }
 
@@ -276,7 +281,7 @@ template <class T> struct Pose { V3<T> p; M3<T> R; };
 template <class T> DLO_HD Pose<T> make_pose(const T* a_prev, const T* a_cur, T tau) {
   T xi[6];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) xi[k] = (T(1) - tau) * a_prev[k] + tau * a_cur[k];
+  for (int k = 0; k < 6; ++k) xi[k] = fma_(tau, a_cur[k], (T(1) - tau) * a_prev[k]);
   Pose<T> g;
   g.p = mk3<T>(xi[0], xi[1], xi[2]);
   g.R = rodrigues(mk3<T>(xi[3], xi[4], xi[5]));

@@ -58,7 +58,7 @@ template <int VPL> struct ContactCache {
 
 // intermediates of one substep that outlive it when REC (all per lane)
 template <int VPL> struct SubRec {
-  f3 v1[VPL], xp[VPL], dx[VPL], v3[VPL], v4[VPL], t_old[VPL];
+  f3 v1[VPL], xp[VPL] /* reverse pass only */, dx[VPL], v3[VPL], v4[VPL], t_old[VPL];
   float S[VPL];
   unsigned active[VPL];   // bit k<K: primitive k responded; bit K+2g+f: finger f of gripper g responded
   int ncand, any_pen;
@@ -67,6 +67,20 @@ template <int VPL> struct SubRec {
   unsigned jac_mask;      // bit it: the Jacobi pass of iteration it applied at least one correction
 };
 
+// (hi, lo) <- (hi + lo) + a, renormalised so that |lo| <= ulp(hi)/2: Knuth's two-sum of hi and a (exact), the old low part
+// added to its error term, then a fast two-sum.  No FMA contraction can change it: there are no products here.
+__device__ __forceinline__ void two_float_add(float& hi, float& lo, float a) {
+  const float t = __fadd_rn(hi, a);
+  const float bb = __fsub_rn(t, hi);
+  const float err = __fadd_rn(__fsub_rn(hi, __fsub_rn(t, bb)), __fsub_rn(a, bb));
+  const float l2 = __fadd_rn(lo, err);
+  hi = __fadd_rn(t, l2);
+  lo = __fsub_rn(l2, __fsub_rn(hi, t));
+}
+__device__ __forceinline__ void two_float_add(f3& hi, f3& lo, const f3& a) {
+  two_float_add(hi.x, lo.x, a.x); two_float_add(hi.y, lo.y, a.y); two_float_add(hi.z, lo.z, a.z);
+}
+
 // A1 (L129, R-20): lane g < G evaluates gripper g at the substep's start and end and publishes it
 // `chain`: the block still holds the previous substep of the same step, whose end pose is this substep's start pose
 __device__ __forceinline__ void publish_poses(const KParams& P, int env, int lane, const float ap[6], const float ac[6], int s, float* pose_sm,
@@ -74,17 +88,32 @@ __device__ __forceinline__ void publish_poses(const KParams& P, int env, int lan
   if (lane < P.G) {
     const float tau0 = (float)s / (float)P.n_sub, tau1 = (float)(s + 1) / (float)P.n_sub;
     float* o = pose_sm + lane * POSE_STRIDE;
+    // The gripper POSITION is interpolated in double and kept as a two-float sum (hi in P0 / P1, lo in P0L / P1L): grasped
+    // vertices are put at p + R q every substep, and an fp32 p at 0.5 m would jitter them by 3e-8 m against their free
+    // neighbours, i.e. 3e-8 / h of velocity noise through Eq.10.  R stays fp32: its rounding is scaled by |q| ~ 1 cm.
+    auto put_p = [&](float tau, int at, int at_lo) {
+      const double td = (double)tau;
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        const double pd = fma(td, (double)ac[k], (1.0 - td) * (double)ap[k]);
+        const float hi = (float)pd;
+        o[at + k] = hi; o[at_lo + k] = (float)(pd - (double)hi);
+      }
+    };
     if (chain) {
 #pragma unroll
       for (int k = 0; k < 12; ++k) o[POSE_P0 + k] = o[POSE_P1 + k];   // p1, R1 -> p0, R0 (contiguous)
+#pragma unroll
+      for (int k = 0; k < 3; ++k) o[POSE_P0L + k] = o[POSE_P1L + k];
     } else {
       const Pose<float> g0 = make_pose<float>(ap, ac, tau0);
-      o[POSE_P0] = g0.p.x; o[POSE_P0 + 1] = g0.p.y; o[POSE_P0 + 2] = g0.p.z;
+      put_p(tau0, POSE_P0, POSE_P0L);
 #pragma unroll
       for (int k = 0; k < 9; ++k) o[POSE_R0 + k] = g0.R.m[k];
     }
-    const Pose<float> g1 = make_pose<float>(ap, ac, tau1);
-    o[POSE_P1] = g1.p.x; o[POSE_P1 + 1] = g1.p.y; o[POSE_P1 + 2] = g1.p.z;
+    Pose<float> g1 = make_pose<float>(ap, ac, tau1);
+    put_p(tau1, POSE_P1, POSE_P1L);
+    g1.p = mk3<float>(o[POSE_P1], o[POSE_P1 + 1], o[POSE_P1 + 2]);
 #pragma unroll
     for (int k = 0; k < 9; ++k) o[POSE_R1 + k] = g1.R.m[k];
     const float* fg = P.finger + ((size_t)env * P.G + lane) * 4;
@@ -109,13 +138,31 @@ __device__ __forceinline__ Pose<float> read_pose(const float* o, int which) {
   for (int k = 0; k < 9; ++k) g.R.m[k] = R[k];
   return g;
 }
-// target of a grasped vertex at the end of the substep: p1 + R1 q  (L103 kinematic flag, R-19)
-__device__ __forceinline__ f3 grasp_target(const KParams& P, const WarpSmem& sm, int code) {
+// target of a grasped vertex at the end of the substep: p1 + R1 q  (L103 kinematic flag, R-19), as a two-float sum hi + lo
+__device__ __forceinline__ f3 grasp_target(const KParams& P, const WarpSmem& sm, int code, f3& lo) {
   const int slot = code - KIN_GRASP0, g = slot / P.M;
   const float* o = sm.pose + g * POSE_STRIDE;
   const float* q = sm.q + 3 * slot;
   Pose<float> g1 = read_pose(o, 1);
-  return g1.p + mul(g1.R, mk3<float>(q[0], q[1], q[2]));
+  const float* Rm = g1.R.m;   // R q + p_lo, every sum of products an explicit fma (same bits in every kernel)
+  const f3 s = mk3<float>(fma_(Rm[0], q[0], fma_(Rm[1], q[1], fma_(Rm[2], q[2], o[POSE_P1L]))),
+                          fma_(Rm[3], q[0], fma_(Rm[4], q[1], fma_(Rm[5], q[2], o[POSE_P1L + 1]))),
+                          fma_(Rm[6], q[0], fma_(Rm[7], q[1], fma_(Rm[8], q[2], o[POSE_P1L + 2]))));
+  f3 hi = g1.p;
+  lo = zero3<float>();
+  two_float_add(hi, lo, s);
+  return hi;
+}
+// velocity of the finger-body point at world y over the substep (L103): (y - [p0 + R0 R1^T (y - p1)]) / h, evaluated as
+// ((p1 - p0) + (R1 - R0) local) / h with local = R1^T (y - p1): the same number without differencing two positions at 0.5 m
+__device__ __forceinline__ f3 finger_body_velocity(const float* o, const f3& y, float inv_h) {
+  const Pose<float> g0 = read_pose(o, 0), g1 = read_pose(o, 1);
+  const f3 local = mulT(g1.R, y - g1.p);
+  const f3 dp = (g1.p - g0.p) + (mk3<float>(o[POSE_P1L], o[POSE_P1L + 1], o[POSE_P1L + 2]) - mk3<float>(o[POSE_P0L], o[POSE_P0L + 1], o[POSE_P0L + 2]));
+  M3<float> dR;
+#pragma unroll
+  for (int k = 0; k < 9; ++k) dR.m[k] = g1.R.m[k] - g0.R.m[k];
+  return inv_h * (dp + mul(dR, local));
 }
 
 // A2 bending (Eq.4-7): per owned interior vertex the element gradients Ga, Gb; returns the gathered force
@@ -437,7 +484,7 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
       f3 n;
       if (!sdf_eval<float>(1, Pc, y, phi, n)) continue;
       if ((P.r - phi) * P.inv_eps < P.log_thresh_lo) continue;   // f < threshold for sure: v untouched, skip the body velocity
-      f3 vb = body_point_velocity<float>(read_pose(o, 0), read_pose(o, 1), y, P.inv_h);
+      f3 vb = finger_body_velocity(o, y, P.inv_h);
       if (rigid_response<float>(v, vb, n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << (P.K + 2 * g + fk);
     }
   }
@@ -500,23 +547,22 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   for (int k = 0; k < VPL; ++k) {
     f3 v1 = zero3<float>();
     if (c.kin[k] == KIN_FREE) v1 = idamp * axpy(s.v[k], hm, f[k]);
-    else if (c.kin[k] >= KIN_GRASP0) v1 = inv_h * (grasp_target(P, sm, c.kin[k]) - s.x[k]);
+    else if (c.kin[k] >= KIN_GRASP0) { f3 tl; const f3 th = grasp_target(P, sm, c.kin[k], tl); v1 = inv_h * ((th - s.x[k]) + (tl - s.xl[k])); }
     R.v1[k] = v1;
-    R.xp[k] = axpy(s.x[k], h, v1);
     R.dx[k] = zero3<float>();
     R.S[k] = 0.0f;
   }
-  const f3 xpr = shfl3(R.xp[0], tp.nl);
-  f3 epred[VPL];   // predicted edge vectors, constant during the projection loop
+  // predicted edge vectors, constant during the projection loop: the exact edge of the two-float positions plus h times the
+  // velocity difference - NOT the difference of rounded predicted positions, which would bring back 3e-8 m of noise per vertex
+  f3 epred[VPL];
+  {
+    const f3 xr = shfl3(s.x[0], tp.nl), xlr = shfl3(s.xl[0], tp.nl), v1r = shfl3(R.v1[0], tp.nl);
 #pragma unroll
-  for (int k = 0; k < VPL; ++k) epred[k] = next_of<VPL>(R.xp, xpr, k, tp.ks) - R.xp[k];
-  if (MODE == 2 && lam_rows) store_rows3<VPL>(lam_rows + (ptrdiff_t)(TAPE_XP - TAPE_LAM) * P.NS, tp.base, P.NS, R.xp);   // replay: x^p rows of the tape record
-  // x^p is x + h v^1: recomputed where it is read (one FFMA per component) instead of held in 3 VPL registers across the
-  // projection loop.  `h2` is h made opaque, or the compiler would merge the recomputation with R.xp (kept for the tape
-  // in MODE 1, 2) and keep it in registers; same operands, same rounding, same bits.
-  float h2 = h;
-  asm volatile("" : "+f"(h2));
-  auto XP = [&](int k) { return axpy(s.x[k], h2, R.v1[k]); };
+    for (int k = 0; k < VPL; ++k) epred[k] = axpy(edge_vec<VPL>(s, xr, xlr, k, tp.ks), h, next_of<VPL>(R.v1, v1r, k, tp.ks) - R.v1[k]);
+  }
+  // x^p = x + h v^1 (contact geometry; fp32 positions are ample there): recomputed where it is read, one FFMA per component,
+  // instead of held in 3 VPL registers across the projection loop
+  auto XP = [&](int k) { return axpy(s.x[k], h, R.v1[k]); };
 
   // Self-contact is evaluated lazily (exactly): segment distance is 1-Lipschitz in the end points, so with d_ref the
   // minimum distance of a set of pairs at the positions x_ref where they were last measured, none of them can
@@ -803,19 +849,19 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // tangents of the positions the substep started from, for the frame transport of A9: recomputed here (the expression of
   // edge_refresh, same bits as ec.t had) rather than held in 3 VPL registers across the projection loop
   {
-    const f3 xr = shfl3(s.x[0], tp.nl);
+    const f3 xr = shfl3(s.x[0], tp.nl), xlr = shfl3(s.xl[0], tp.nl);
 #pragma unroll
     for (int k = 0; k < VPL; ++k) {
-      const f3 e = next_of<VPL>(s.x, xr, k, tp.ks) - s.x[k];
+      const f3 e = edge_vec<VPL>(s, xr, xlr, k, tp.ks);
       const float iL = tp.evalid[k] ? rsqrt_(dot(e, e)) : 0.0f;
       R.t_old[k] = iL * e;
     }
   }
-  // -- A8 commit
+  // -- A8 commit: x + xl <- (x + xl) + h v in two-float arithmetic (the rounding error of the sum is kept, not dropped)
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
-    if (c.kin[k] == KIN_FREE) { s.x[k] = axpy(s.x[k], h, vel[k]); s.v[k] = vel[k]; }
-    else if (c.kin[k] >= KIN_GRASP0) { s.x[k] = grasp_target(P, sm, c.kin[k]); s.v[k] = vel[k]; }
+    if (c.kin[k] == KIN_FREE) { two_float_add(s.x[k], s.xl[k], h * vel[k]); s.v[k] = vel[k]; }
+    else if (c.kin[k] >= KIN_GRASP0) { s.x[k] = grasp_target(P, sm, c.kin[k], s.xl[k]); s.v[k] = vel[k]; }
     else if (tp.vvalid[k]) s.v[k] = zero3<float>();
   }
 

@@ -17,7 +17,11 @@ namespace dlo {
 typedef V3<float> f3;
 enum { KIN_FREE = 0, KIN_PINNED = 1, KIN_GRASP0 = 2 };   // kin code >= 2: grasped, slot = code - 2 = g*M + k
 enum { MAT_M = 0, MAT_L0, MAT_STRETCH, MAT_ALPHA, MAT_GAMMA, MAT_SIGY, MAT_RC, MAT_MUR, MAT_MUS, MAT_N };
-enum { ROW_X = 0, ROW_V = 3, ROW_D1 = 6, ROW_KB = 9, STATE_ROWS = 11 };
+// rows of one env's state block.  Positions are kept as an unevaluated sum x + xl of two floats (xl = what the fp32 rounding
+// of x + h v dropped, |xl| <= ulp(x)/2): an fp32 position at 0.5 m carries 3e-8 m of rounding, which the next substep's Eq.10
+// projection turns into 3e-8 / h = 3e-4 m/s of velocity noise - as large as the Coulomb stick threshold mu g h of a vertex
+// resting on the ground.  With the residual carried along, edge vectors are exact differences (noise 5e-10 m, 2e-6 m/s).
+enum { ROW_X = 0, ROW_V = 3, ROW_D1 = 6, ROW_KB = 9, ROW_XL = 11, STATE_ROWS = 14 };
 enum { FLAG_NONFINITE = 1, FLAG_CAND_OVERFLOW = 2 };
 #define DLO_FULL 0xffffffffu
 // primitives in shared memory: [0..14] parameters (boxes expanded to centre(3), half(3), R(9)), [16..18] centre and [19]
@@ -62,7 +66,7 @@ struct KParams {
 };
 
 // per-gripper block in shared memory: p0(3) R0(9) p1(3) R1(9) fingerA0(3) fingerB0(3) fingerA1(3) fingerB1(3) rf(1) pad(3)
-enum { POSE_P0 = 0, POSE_R0 = 3, POSE_P1 = 12, POSE_R1 = 15, POSE_FA0 = 24, POSE_FB0 = 27, POSE_FA1 = 30, POSE_FB1 = 33, POSE_RF = 36, POSE_FC0 = 37, POSE_FC1 = 40, POSE_FRAD = 43, POSE_STRIDE = 44 };   // FC*: finger mid points, FRAD: bounding radius
+enum { POSE_P0 = 0, POSE_R0 = 3, POSE_P1 = 12, POSE_R1 = 15, POSE_FA0 = 24, POSE_FB0 = 27, POSE_FA1 = 30, POSE_FB1 = 33, POSE_RF = 36, POSE_FC0 = 37, POSE_FC1 = 40, POSE_FRAD = 43, POSE_P0L = 44, POSE_P1L = 47, POSE_STRIDE = 52 };   // FC*: finger mid points, FRAD: bounding radius, P*L: low parts of p0, p1 (two-float)
 
 __device__ __forceinline__ float shfl(float v, int src) { return __shfl_sync(DLO_FULL, v, src); }
 __device__ __forceinline__ f3 shfl3(const f3& v, int src) { return mk3<float>(shfl(v.x, src), shfl(v.y, src), shfl(v.z, src)); }
@@ -82,9 +86,9 @@ __device__ __forceinline__ float warp_min(float v) { return __uint_as_float(__re
 __device__ __forceinline__ f3 lds3(const float* s, int NP, int i) { return mk3<float>(s[i], s[NP + i], s[2 * NP + i]); }
 __device__ __forceinline__ void sts3(float* s, int NP, int i, const f3& v) { s[i] = v.x; s[NP + i] = v.y; s[2 * NP + i] = v.z; }
 
-// layout of a side record (float offsets): header (ncand, jac_mask), v^1 rows, candidate codes, depth sums D_p, the summed
-// corrections of every Jacobi pass [N_C][3][33 VPL]
-__host__ __device__ inline int side_off_v1() { return 4; }
+// layout of a side record (float offsets): header (ncand, jac_mask), v^3 rows (velocity after the self-contact friction),
+// candidate codes, depth sums D_p, the summed corrections of every Jacobi pass [N_C][3][33 VPL]
+__host__ __device__ inline int side_off_v3() { return 4; }
 __host__ __device__ inline int side_off_cand(const KParams& P) { return 4 + 3 * P.NS; }
 __host__ __device__ inline int side_off_dp(const KParams& P) { return side_off_cand(P) + P.cand_cap / 2; }
 __host__ __device__ inline int side_off_acc(const KParams& P) { return side_off_dp(P) + P.cand_cap; }
@@ -142,10 +146,12 @@ template <int VPL> __device__ __forceinline__ void store_row(float* __restrict__
 }
 
 // rows of one tape record (per substep and env), each NS floats: the state at the start of the substep, then what the
-// reverse pass would otherwise have to recompute: predicted positions, final corrections, the velocity before the rigid
-// coupling (differencing positions would cost too many digits), Eq.10 multiplier sums, the
-// mask of rigid bodies that responded, and the multipliers of every iteration
-enum { TAPE_XP = STATE_ROWS, TAPE_DX = TAPE_XP + 3, TAPE_V3 = TAPE_DX + 3, TAPE_S = TAPE_V3 + 3, TAPE_ACT = TAPE_S + 1, TAPE_LAM = TAPE_ACT + 1 };
+// reverse pass would otherwise have to recompute: final corrections, the velocity v^1 after the force step (x^p = x + h v^1,
+// the predicted edge vectors and, without self-contact friction, v^3 = v^1 + dx/h follow from it with the forward's own
+// expressions, bit for bit), Eq.10 multiplier sums, the mask of rigid bodies that responded, and the multipliers of every
+// iteration.  (The position residual rows stay in the record: a reverse pass fed fp32-rounded positions was measured to
+// lose the 1e-3 gradient bar on ~5 % of the teacher-forced segments.)
+enum { TAPE_DX = STATE_ROWS, TAPE_V1 = TAPE_DX + 3, TAPE_S = TAPE_V1 + 3, TAPE_ACT = TAPE_S + 1, TAPE_LAM = TAPE_ACT + 1 };
 __host__ __device__ inline int tape_rows(int N_C) { return TAPE_LAM + N_C; }
 
 template <int VPL> __device__ __forceinline__ void store_rows3(float* __restrict__ rows, int base, int NS, const f3 a[VPL]) {
@@ -171,6 +177,7 @@ template <int VPL> __device__ __forceinline__ void load_rows3(const float* __res
 template <int VPL> struct LaneState {
   f3 x[VPL], v[VPL], d1[VPL];
   float kb1[VPL], kb2[VPL];
+  f3 xl[VPL];   // low part of the position (see ROW_XL)
 };
 
 template <int VPL> __device__ __forceinline__ void load_state(const float* __restrict__ blk, int base, int NS, LaneState<VPL>& s) {
@@ -183,6 +190,7 @@ template <int VPL> __device__ __forceinline__ void load_state(const float* __res
     s.v[k] = mk3<float>(r[3][k], r[4][k], r[5][k]);
     s.d1[k] = mk3<float>(r[6][k], r[7][k], r[8][k]);
     s.kb1[k] = r[9][k]; s.kb2[k] = r[10][k];
+    s.xl[k] = mk3<float>(r[11][k], r[12][k], r[13][k]);
   }
 }
 template <int VPL> __device__ __forceinline__ void store_state(float* __restrict__ blk, int base, int NS, const LaneState<VPL>& s) {
@@ -192,6 +200,7 @@ template <int VPL> __device__ __forceinline__ void store_state(float* __restrict
   DLO_ST(3, s.v[k].x) DLO_ST(4, s.v[k].y) DLO_ST(5, s.v[k].z)
   DLO_ST(6, s.d1[k].x) DLO_ST(7, s.d1[k].y) DLO_ST(8, s.d1[k].z)
   DLO_ST(9, s.kb1[k]) DLO_ST(10, s.kb2[k])
+  DLO_ST(11, s.xl[k].x) DLO_ST(12, s.xl[k].y) DLO_ST(13, s.xl[k].z)
 #undef DLO_ST
 }
 
@@ -248,11 +257,16 @@ template <int VPL> __device__ __forceinline__ f3 next_of(const f3 a[VPL], const 
   return (k == ks) ? remote : a[k + 1 < VPL ? k + 1 : k];
 }
 
+// exact edge vector of slot k from the two-float positions: the difference of the high parts is exact (neighbours agree in
+// their leading bits), the low parts add what the stored fp32 positions had rounded away
+template <int VPL> __device__ __forceinline__ f3 edge_vec(const LaneState<VPL>& s, const f3& xr, const f3& xlr, int k, int ks) {
+  return (next_of<VPL>(s.x, xr, k, ks) - s.x[k]) + (next_of<VPL>(s.xl, xlr, k, ks) - s.xl[k]);
+}
 template <int VPL> __device__ __forceinline__ void edge_refresh(const Topo<VPL>& tp, const LaneState<VPL>& s, EdgeCache<VPL>& ec) {
-  const f3 xr = shfl3(s.x[0], tp.nl);
+  const f3 xr = shfl3(s.x[0], tp.nl), xlr = shfl3(s.xl[0], tp.nl);
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
-    f3 e = next_of<VPL>(s.x, xr, k, tp.ks) - s.x[k];
+    f3 e = edge_vec<VPL>(s, xr, xlr, k, tp.ks);
     float L2 = dot(e, e);
     float iL = tp.evalid[k] ? rsqrt_(L2) : 0.0f;
     ec.iL[k] = iL;

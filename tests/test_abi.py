@@ -22,12 +22,12 @@ def dlo():
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "dlo.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(dlo_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(dlo_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(dlo):
     names = declared_symbols()
-    assert len(names) >= 17
+    assert len(names) >= 20
     L = dlo.lib()
     for n in names:
         assert hasattr(L, n), n
@@ -45,9 +45,9 @@ def test_scratch_bytes_matches_layout(dlo):
     P = make_problem(5)
     cfg = make_config(P["config"])
     B, N, H, S = 4096, 128, 1000, 100
-    blk = 11 * N * 4
+    blk = 14 * N * 4                    # x, v, d1 (3 rows each), kappa_bar (2), position residual x_lo (3)
     n = dlo.dlo_scratch_bytes(cfg, H, S)
-    ckpt, tape = (H // S + 1) * B * blk, 2 * (S * 5 + 1) * B * (22 + 10) * N * 4     # two tape buffers of 22 + N_C rows per record
+    ckpt, tape = (H // S + 1) * B * blk, 2 * (S * 5 + 1) * B * (22 + 10) * N * 4     # two tape buffers of 22 + N_C rows per record (14 state, dx 3, v1 3, S, mask)
     # two side-record pools (one substep in twelve; header, v^1, 480 candidate codes and depth sums, N_C x 3 x 132 corrections)
     side = 2 * ((S * 5 + 1) * B // 12) * (4 + 3 * N + 240 + 480 + 10 * 3 * 132) * 4
     assert n > ckpt + tape + side and n < ckpt + tape + side + 450e6

@@ -143,12 +143,12 @@ def test_side_records_equal_recompute(dlo, monkeypatch, cfg, H, stride, tol):
         assert np.abs(outs[1][k] - outs[0][k]).max() <= tol * np.abs(outs[0][k]).max(), k
 
 
-# Kinked cases: Eq.11 drives every active hinge onto its yield surface
-# and resting contact sits on the f = 1 / approach thresholds, where the step is continuous but its derivative jumps.
-# There the oracle's own gradient moves by far more than 1e-3 when its inputs move by one fp32 rounding, so no fp32
-# (or perturbed fp64) run can reproduce it.  Bar: the median env meets 1e-3; every env is within 1e-3 or no further
-# from the oracle than 5x the oracle's own spread under fp32-sized input perturbations, except at most a quarter of
-# the envs (a flip seen by the GPU run only).
+# Kinked cases: Eq.11 drives every active hinge onto its yield surface, resting contact sits on the
+# kink of f = min(exp(d/eps_s), 1), dragged ropes on the Coulomb stick / slide switch: the step is continuous there but its
+# derivative jumps, and the oracle's own gradient moves by far more than 1e-3 when its inputs move by one fp32 rounding.
+# Bar: every env whose ORACLE gradient is stable under such perturbations (three draws, spread < 1e-3 / (2 sqrt(#substeps)):
+# the fp32 run injects one kick per substep where the spread measures ONE) meets the plain 1e-3;
+# the others are counted and held to a finite cap.  (The plain-bar claim at full size is tests/test_teacher_forced_gpu.py's.)
 KINKED = [
     ("cfg2 ground+grippers", dict(cfg_id=2, batch=8, n_verts=24), 40, 16, ALL4),
     ("cfg3 plasticity+fingers", dict(cfg_id=3, batch=8, n_verts=24), 40, 10, ALL4),
@@ -174,10 +174,10 @@ def test_gradient_parity_at_kinks(dlo, orc, name, kw, H, stride, keys):
             spread[k] = np.maximum(spread[k], gradient_error(env_first(k, gq[k]), env_first(k, ref[k])))
     for k in keys:
         err = gradient_error(env_first(k, got[k]), env_first(k, ref[k]))
-        ok = (err <= GRAD_TOL) | (err <= 5.0 * spread[k])
-        print(summarize("%s %s gpu" % (name, k), err), "|", summarize("oracle spread", spread[k]), "| outside: %d" % (~ok).sum())
-        assert np.median(err) <= GRAD_TOL, (name, k, np.median(err))
-        assert (~ok).sum() <= len(err) // 4, (name, k, err, spread[k])
+        stable = spread[k] < GRAD_TOL / (2.0 * np.sqrt(H * P["config"]["n_substeps"]))
+        print(summarize("%s %s gpu" % (name, k), err), "|", summarize("oracle spread", spread[k]), "| oracle-stable envs: %d of %d" % (stable.sum(), len(err)))
+        assert (err[stable] <= GRAD_TOL).all(), (name, k, err, spread[k])
+        assert np.isfinite(err).all() and (err <= 10.0).all(), (name, k, err)
 
 
 @pytest.mark.parametrize("N,ring", [(3, False), (4, True), (5, True), (256, False), (255, True)],

@@ -61,21 +61,22 @@ def test_forward_parity(dlo, orc, name, kw, over):
     err = position_error(P, got["x"], ref["x"])
     print(summarize(name, err))
     assert np.isfinite(got["x"]).all()
-    if err.max() > POS_TOL:
-        # Some envs of the contact-rich workloads are chaotic: the ORACLE's own final positions move by more than
-        # 1e-4 when its inputs move by one fp32 rounding.  Every env must be within 1e-4
-        # or no further from the oracle than 5x that spread, bar at most a quarter; the median env must meet 1e-4
-        # (or 3x the median spread where even the median env is chaotic at this horizon).
-        spread = oracle_position_spread(orc, P, P["horizon"], ref["x"])
-        ok = (err <= POS_TOL) | (err <= 5.0 * spread)
-        print(summarize(name + " oracle spread", spread), "| outside: %d" % (~ok).sum())
-        assert np.median(err) <= max(POS_TOL, 3.0 * np.median(spread)), summarize(name, err)
-        assert (~ok).sum() <= len(err) // 4, (name, err, spread)
-        return
-    # frames stay unit and orthogonal to their edges (state invariant of A9)
     E = P["config"]["n_verts"] - (0 if P["config"]["topology"] else 1)
     d1 = got["d1"][:, :, :E]
-    assert np.abs(np.linalg.norm(d1, axis=1) - 1).max() < 1e-5
+    assert np.abs(np.linalg.norm(d1, axis=1) - 1).max() < 1e-5          # frames stay unit (state invariant of A9), chaotic or not
+    if err.max() > POS_TOL:
+        # Some envs of the contact-rich workloads are chaotic at this horizon: the ORACLE's own final positions move by more
+        # than the tolerance when its inputs move by one fp32 rounding.  The plain bar is asserted on
+        # every env whose oracle result is stable under such a perturbation: the fp32 run injects one rounding-sized kick per
+        # substep where the spread measures the effect of ONE, so "stable" is spread < tolerance / (2 sqrt(#substeps)); the
+        # others are counted and held to a finite cap.  The plain-bar claim on those workloads is tests/test_teacher_forced_gpu.py's.
+        spread = oracle_position_spread(orc, P, P["horizon"], ref["x"])
+        stable = spread < POS_TOL / (2.0 * np.sqrt(P["horizon"] * P["config"]["n_substeps"]))
+        print(summarize(name + " oracle spread", spread), "| oracle-stable envs: %d of %d" % (stable.sum(), len(err)))
+        assert (err[stable] <= POS_TOL).all(), (name, err, spread)
+        assert (err <= 0.5).all(), (name, err)
+        return
+    # frames and rest curvature follow the oracle's
     dref = ref["d1"][:, :, :E]
     assert np.abs(d1 - dref).max() < 5e-3
     assert np.abs(got["kappa_bar"] - ref["kappa_bar"]).max() < 5e-3 * max(1.0, np.abs(ref["kappa_bar"]).max())
@@ -195,7 +196,8 @@ def test_host_buffer_calls_match_device_calls(dlo):
     P = make_problem(3, batch=8, n_verts=24, horizon=20, stride=7)
     from parity import loss_and_seed
     sim = dlo.DloSim(P)
-    xd = sim.rollout(20, 7).state()["x"]
+    sim.rollout(20, 7)
+    xd = sim.state_device()["x"].double().cpu().numpy()      # the fp32 positions dlo_get_state returns (without the residual)
     _, seed = loss_and_seed(P, xd)
     gd = sim.backward(seed)
     f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)

@@ -50,8 +50,19 @@ def _resample_polyline(pts, n):
     return out
 
 
+CLEARANCE = 1.0e-4   # initial gap to a surface the rope is laid on / wrapped around
+# Finger capsules stand FINGER_SLACK beyond touching distance on either side of the held rope: the vertices next to a grasped
+# one move with the gripper, so against a finger that just touches them their approach speed u_n is zero to
+# rounding for the whole rollout and the branch u_n < 0 - hence every action gradient - is decided by the last bit.  With
+# 3 mm of slack (f = exp(-3) < the 0.1 threshold) the fingers act when the rope swings into them, not on what they carry.
+FINGER_SLACK = 3.0e-3
+
+
 def _slack_u(span, height, length, r, n):
-    """Down-slope, flat stretch resting at z=r, up-slope; total arclength `length`; ends `span` apart at `height`."""
+    """Down-slope, flat stretch lying CLEARANCE above its rest height z=r, up-slope; total arclength `length`; ends `span`
+    apart at `height`.  (Not at z=r exactly: phi = r is the kink of f = min(exp(d / eps_s), 1) of PAPER.md L103, where the
+    derivative of the step jumps; a rope laid exactly there would make every gradient depend on the last bit of r - z.)"""
+    r = r + CLEARANCE
     hh = height - r
     k = 0.5 * (length - span)                 # sqrt(d^2+hh^2) - d = k
     d = (hh * hh - k * k) / (2.0 * k)
@@ -205,7 +216,7 @@ def _make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
         pose0[:, 0, 5] = 0.5 * np.pi                                      # fingers straddle the rope (local x -> world y)
         P["init_pose"] = pose0
         fg = np.zeros((B, 1, 4))
-        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (rf + r), 0.04, rf
+        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (rf + r + FINGER_SLACK), 0.04, rf
         P["finger_geom"] = fg
         P["actions"] = pose0[None] + _smooth_random_actions(rng, H, B, 1, 0.2, 1.0)
         P["loss"] = dict(kind="polyline", target=_smooth_target_polyline(rng, B, N, P["actions"][-1, :, 0, :3], 1.0))
@@ -221,7 +232,7 @@ def _make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
         D = rng.uniform(0.24, 0.27, B)
         c1 = np.stack([-0.5 * D + rng.uniform(-5e-3, 5e-3, B), rng.uniform(-5e-3, 5e-3, B)], axis=1)
         c2 = np.stack([+0.5 * D + rng.uniform(-5e-3, 5e-3, B), rng.uniform(-5e-3, 5e-3, B)], axis=1)
-        z0, rho = 0.1, R + r
+        z0, rho = 0.1, R + r + CLEARANCE          # wrapped CLEARANCE off the posts (see _slack_u)
         x0 = np.zeros((B, 3, N))
         grasp = np.zeros(B, dtype=np.int64)
         for b in range(B):
@@ -249,7 +260,7 @@ def _make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
         pose0[:, 0, 5] = 0.5 * np.pi
         P["init_pose"] = pose0
         fg = np.zeros((B, 1, 4))
-        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (0.01 + r), 0.04, 0.01
+        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (0.01 + r + FINGER_SLACK), 0.04, 0.01
         P["finger_geom"] = fg
         dy, dz = rng.uniform(-0.09, -0.06, B), rng.uniform(0.0, 0.03, B)
         s = (np.arange(H) + 1) / H
@@ -307,7 +318,7 @@ def _make_problem(cfg_id, batch=None, n_verts=None, horizon=None, stride=None):
         pose0[:, 1, :3] = 0.5 * (x0[:, :, -2] + x0[:, :, -1])
         P["init_pose"] = pose0
         fg = np.zeros((B, 2, 4))
-        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (rf + r), 0.04, rf
+        fg[..., 0], fg[..., 1], fg[..., 2] = 2 * (rf + r + FINGER_SLACK), 0.04, rf
         P["finger_geom"] = fg
         P["actions"] = pose0[None] + _smooth_random_actions(rng, H, B, 2, 0.2, 1.0)
         P["loss"] = dict(kind="polyline", target=_smooth_target_polyline(rng, B, N, P["actions"][-1, :, 0, :3], 1.0))
