@@ -101,7 +101,15 @@ static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 static int smem_layout(KParams& P, int VPL, bool adjoint) {
   const int NP = 33 * VPL;   // padded row (vpos)
   int o = 0;
-  auto take = [&](int n) { int at = o; o += round_up(n, 4); return at; };
+  P.n_guard = 0;
+  // DLO_CHECKS=1 (the pool's compute-sanitizer being closed): four guard words behind every region, filled by warp_setup and
+  // verified when the kernel ends (FLAG_GUARD); aliased views (sm_blk, sm_xref in the adjoint) share their host region's guard
+  auto take = [&](int n) {
+    int at = o;
+    o += round_up(n, 4);
+    if (P.checks && n > 0 && P.n_guard < 24) { P.sm_guard[P.n_guard++] = o; o += 4; }
+    return at;
+  };
   P.sm_pose = take(P.G * POSE_STRIDE);
   P.sm_prim = take(P.K * PRIM_SM_STRIDE);
   P.sm_q = take(P.G * P.M * 3);
@@ -164,6 +172,7 @@ static void fill_params(const dlo_config& c, KParams& P) {
   for (int k = 0; k < 3; ++k) P.g[k] = c.gravity[k];
   P.r = c.rope_radius; P.inv_eps = 1.0f / c.contact_softness; P.f_thresh = c.influence_threshold; P.e_rest = c.restitution;
   P.log_thresh_lo = logf(c.influence_threshold) - 0.01f;
+  if (const char* ov = getenv("DLO_CHECKS")) P.checks = atoi(ov);   // 1: checks on; 2: and a deliberate overrun (self-test of the check)
 }
 
 size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
@@ -188,7 +197,14 @@ size_t dlo_scratch_bytes(const dlo_config* c, int32_t horizon, int32_t stride) {
   return n;
 }
 
-template <class T> static cudaError_t dalloc(T** p, size_t n) { return cudaMalloc((void**)p, (n ? n : 1) * sizeof(T)); }
+// DLO_CHECKS=1: every library allocation starts as 0xff bytes (NaN as a float, -1 as an int), so that a read of memory
+// nothing wrote shows up in the results (the stand-in for compute-sanitizer's initcheck, closed on this pool)
+static bool checks_on() { const char* v = getenv("DLO_CHECKS"); return v && atoi(v) != 0; }
+template <class T> static cudaError_t dalloc(T** p, size_t n) {
+  cudaError_t e = cudaMalloc((void**)p, (n ? n : 1) * sizeof(T));
+  if (e == cudaSuccess && checks_on()) e = cudaMemset(*p, 0xff, (n ? n : 1) * sizeof(T));
+  return e;
+}
 
 extern "C" {
 
@@ -573,9 +589,11 @@ dlo_status dlo_check_numerics(dlo_sim* s, int32_t* n_bad) {
   CU(cudaMemcpyAsync(f.data(), s->flags, f.size() * sizeof(int), cudaMemcpyDeviceToHost, s->stream));
   CU(cudaStreamSynchronize(s->stream));
   int bad = 0, ovf = 0;
-  for (int v : f) { bad += v != 0; ovf += (v & FLAG_CAND_OVERFLOW) != 0; }
+  int grd = 0;
+  for (int v : f) { bad += v != 0; ovf += (v & FLAG_CAND_OVERFLOW) != 0; grd += (v & FLAG_GUARD) != 0; }
   if (n_bad) *n_bad = bad;
-  if (bad) return fail(DLO_ERR_NUMERIC, std::to_string(bad) + " env(s) flagged (" + std::to_string(ovf) + " self-contact candidate overflow, rest non-finite)");
+  if (bad) return fail(DLO_ERR_NUMERIC, std::to_string(bad) + " env(s) flagged (" + std::to_string(ovf) + " self-contact candidate overflow, " +
+                                            std::to_string(grd) + " shared-memory guard, rest non-finite)");
   return DLO_OK;
 }
 

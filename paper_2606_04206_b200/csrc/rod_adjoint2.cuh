@@ -487,6 +487,7 @@ __global__ void __launch_bounds__(DLO_ADJ_WARPS * 32, 1) k_adjoint(const __grid_
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(DLO_FULL, v, o);
     if (tp.lane == 0) P.gmat[(size_t)env * 5 + k] += (float)v;
   }
+  verify_guards(P, env, tp.lane, sm);
 }
 
 // seeds of the reverse pass -> running adjoint block; gradients out of it

@@ -166,6 +166,10 @@ __device__ __forceinline__ void warp_setup(const KParams& P, int env, int lane, 
     else if (ty == 3) dst[PRIM_BR] = sqrt_(src[3] * src[3] + src[4] * src[4] + src[5] * src[5]);
   }
   for (int k = lane; k < P.G * P.M * 3; k += 32) sm.q[k] = P.qloc[(size_t)env * P.G * P.M * 3 + k];
+  if (P.checks)
+    for (int k = lane; k < 4 * P.n_guard; k += 32) reinterpret_cast<unsigned*>(sm.base)[P.sm_guard[k >> 2] + (k & 3)] = DLO_GUARD_WORD;
+  __syncwarp();
+  if (P.checks == 2 && P.K > 0 && lane == 0) sm.prim[P.K * PRIM_SM_STRIDE] = 0.0f;   // self-test of the check: one word past the primitives
   if (P.self_contact)
     for (int k = lane; k < 3 * sm.NP; k += 32) sm.acc[k] = 0.0f;
   __syncwarp();
@@ -197,6 +201,15 @@ __global__ void __launch_bounds__(1024, 1) k_sort_envs(int B, const int* __restr
   }
   __syncthreads();
   for (int i = tid; i < B; i += 1024) perm[atomicAdd(&hist[min(max(stat[2 * i + col] >> shift, 0), 1023)], 1)] = i;
+}
+
+// DLO_CHECKS: every guard word behind the warp's shared-memory regions must still be there
+__device__ __forceinline__ void verify_guards(const KParams& P, int env, int lane, const WarpSmem& sm) {
+  if (!P.checks) return;
+  __syncwarp();
+  bool bad = false;
+  for (int k = lane; k < 4 * P.n_guard; k += 32) bad |= reinterpret_cast<const unsigned*>(sm.base)[P.sm_guard[k >> 2] + (k & 3)] != DLO_GUARD_WORD;
+  if (__any_sync(DLO_FULL, bad) && lane == 0) atomicOr(P.flags + env, FLAG_GUARD);
 }
 
 template <int VPL> __device__ __forceinline__ bool state_finite(const LaneState<VPL>& s) {
@@ -278,6 +291,7 @@ __global__ void __launch_bounds__(DLO_FWD_WARPS * 32, VPL <= 4 ? 2 : 1) k_forwar
   if (P.stat && tp.lane == 0) { P.stat[2 * env] = work; P.stat[2 * env + 1] = npen; }
   const bool ok = state_finite<VPL>(s);
   if (__any_sync(DLO_FULL, !ok) && tp.lane == 0) atomicOr(P.flags + env, FLAG_NONFINITE);
+  verify_guards(P, env, tp.lane, sm);
 }
 
 }  // namespace dlo

@@ -22,7 +22,8 @@ enum { MAT_M = 0, MAT_L0, MAT_STRETCH, MAT_ALPHA, MAT_GAMMA, MAT_SIGY, MAT_RC, M
 // projection turns into 3e-8 / h = 3e-4 m/s of velocity noise - as large as the Coulomb stick threshold mu g h of a vertex
 // resting on the ground.  With the residual carried along, edge vectors are exact differences (noise 5e-10 m, 2e-6 m/s).
 enum { ROW_X = 0, ROW_V = 3, ROW_D1 = 6, ROW_KB = 9, ROW_XL = 11, STATE_ROWS = 14 };
-enum { FLAG_NONFINITE = 1, FLAG_CAND_OVERFLOW = 2 };
+enum { FLAG_NONFINITE = 1, FLAG_CAND_OVERFLOW = 2, FLAG_GUARD = 4 /* DLO_CHECKS: a shared-memory region was written past its end */ };
+#define DLO_GUARD_WORD 0x7fc0dead   /* a NaN bit pattern no computation produces */
 #define DLO_FULL 0xffffffffu
 // primitives in shared memory: [0..14] parameters (boxes expanded to centre(3), half(3), R(9)), [16..18] centre and [19]
 // radius of a bounding sphere (radius < 0: unbounded, e.g. a plane) used to cull vertices that are out of reach
@@ -31,6 +32,8 @@ enum { PRIM_NP = 10, PRIM_SM_STRIDE = 20, PRIM_BC = 16, PRIM_BR = 19 };
 struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
   int G, M, K, cand_cap, hot_cap;
+  int checks;            // DLO_CHECKS=1: guard words behind every per-warp shared-memory region, verified when a kernel ends
+  int n_guard, sm_guard[24];   // their positions (float offsets from the warp's base)
   int t_base;            // frame index of the rollout's first step: step t of the launch uses actions[t_base + t - 1], actions[t_base + t]
   float h, inv_h, g[3], r, inv_eps, f_thresh, e_rest, log_thresh_lo /* log(f_thresh) - 0.01 */;
   int vote_mode;         // bit 0: the warps of a CTA refresh their contact data together; bit 1: ... and rebuild their pair lists together

@@ -3,10 +3,15 @@ uninitialised memory would hide (SURVEY.md section 5 "Race detection"): self-con
 recomputing reverse pass (no side-record pool), pair-list rebuilds in the middle of the projection loop, odd rings (third
 colour), aliased shared-memory regions (block spheres on sm.vs, xref on ybar), gripper fingers and boxes.
 
-They run in the normal GPU suite (results finite, flags clear, repeatable bits) and are the workload of the
-compute-sanitizer runs whose summaries are under profiles/ (memcheck, racecheck, synccheck, initcheck):
-
-    compute-sanitizer --tool <tool> python -m pytest tests/test_sanitizer_cases_gpu.py -x -q
+compute-sanitizer is CLOSED on this GPU pool (the tool answers: "compute-sanitizer is closed on this pool and stays closed:
+runs under it have left GPUs needing a reset. Find a bad access with bounds checks and asserts of your own, small cases,
+and a comparison with the CPU reference"; profiles/r02_sanitizer.md).  The stand-ins, all in this file:
+  - every case runs twice and must give identical forward bits (a data race shows as a difference sooner or later), under
+    different CTA shapes and vote modes elsewhere (test_parity_gpu.py::test_lazy_self_contact_schedule_changes_no_bit);
+  - every case also runs with DLO_CHECKS=1: four guard words behind every per-warp shared-memory region, verified when a
+    kernel ends (an overrun sets FLAG_GUARD -> DLO_ERR_NUMERIC), and every library allocation pre-filled with 0xff bytes
+    (NaN / -1), so that a read of memory nothing wrote ends up in a non-finite result or a wild index (memcheck / initcheck);
+  - results are compared with the fp64 oracle by the parity tests on the same paths.
 """
 import numpy as np
 import pytest
@@ -24,6 +29,15 @@ def dlo():
     import paper_2606_04206_b200 as pkg
     pkg.lib()
     return pkg
+
+
+@pytest.fixture(autouse=True, params=[0, 1], ids=["plain", "DLO_CHECKS"])
+def checks(request, monkeypatch):
+    if request.param:
+        monkeypatch.setenv("DLO_CHECKS", "1")
+    else:
+        monkeypatch.delenv("DLO_CHECKS", raising=False)
+    return request.param
 
 
 def fwd_bwd(dlo, P, H, stride):
@@ -84,3 +98,16 @@ def test_full_feature_set_small(dlo):
     twice(dlo, make_problem(5, batch=5, n_verts=40, horizon=6, stride=3), 6, 3)
     twice(dlo, make_problem(4, batch=3, n_verts=48, horizon=6, stride=4), 6, 4)
     twice(dlo, make_problem(3, batch=3, n_verts=24, horizon=6, stride=2), 6, 2)
+
+
+def test_the_guard_check_can_fail(dlo, monkeypatch):
+    """DLO_CHECKS=2 makes every warp write one word past its primitive block: every env must come back flagged"""
+    import ctypes as C
+    monkeypatch.setenv("DLO_CHECKS", "2")
+    P = make_problem(5, batch=5, n_verts=40, horizon=2, stride=0)
+    sim = dlo.DloSim(P)
+    sim.rollout(2, 0)
+    n = C.c_int32(0)
+    assert dlo.lib().dlo_check_numerics(sim.h, C.byref(n)) == -6 and n.value == 5
+    assert "5 shared-memory guard" in dlo.dlo_last_error()
+    sim.close()
