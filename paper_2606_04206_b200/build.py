@@ -4,7 +4,8 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libdlo_b200.so")
+# DLO_B200_LIB / DLO_NVCC_EXTRA: development variants (another output file, extra nvcc flags); the product is libdlo_b200.so
+LIB = os.environ.get("DLO_B200_LIB") or os.path.join(HERE, "libdlo_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v",
@@ -31,7 +32,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB + ".tmp", os.path.join(CSRC, "dlo_api.cu")]
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("DLO_NVCC_EXTRA", "").split() + ["-o", LIB + ".tmp", os.path.join(CSRC, "dlo_api.cu")]
         r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
         if verbose or r.returncode != 0:
             print(r.stdout + r.stderr)

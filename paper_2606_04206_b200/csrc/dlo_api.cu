@@ -172,6 +172,8 @@ static void fill_params(const dlo_config& c, KParams& P) {
   for (int k = 0; k < 3; ++k) P.g[k] = c.gravity[k];
   P.r = c.rope_radius; P.inv_eps = 1.0f / c.contact_softness; P.f_thresh = c.influence_threshold; P.e_rest = c.restitution;
   P.log_thresh_lo = logf(c.influence_threshold) - 0.01f;
+  P.phase_mask = 0xffffffffu;
+  if (const char* ov = getenv("DLO_PHASES")) P.phase_mask = (unsigned)strtoul(ov, nullptr, 0);   // tuning override (no effect on results)
   if (const char* ov = getenv("DLO_CHECKS")) P.checks = atoi(ov);   // 1: checks on; 2: and a deliberate overrun (self-test of the check)
 }
 

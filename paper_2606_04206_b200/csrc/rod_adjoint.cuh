@@ -68,7 +68,7 @@ struct GraspAcc {
     g = -1;
   }
   __device__ __forceinline__ void add(const KParams& P, const WarpSmem& sm, int code, const f3& tbar) {
-    const int slot = code - KIN_GRASP0, gg = slot / P.M;
+    const int slot = code - KIN_GRASP0, gg = (slot >= P.M) + (slot >= 2 * P.M) + (slot >= 3 * P.M);
     if (gg != g) { flush(sm); pose_bar_zero(b); g = gg; }
     const float* q = sm.q + 3 * slot;
     rigid_point_adj<float>(mk3<float>(q[0], q[1], q[2]), tbar, b);

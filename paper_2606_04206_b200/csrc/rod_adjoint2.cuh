@@ -122,7 +122,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
 #pragma unroll
   for (int k = 0; k < VPL; ++k) { tbar_old[k] = zero3<float>(); tbar_new[k] = zero3<float>(); }
 
-  phase_sync(sm);
+  phase_sync(sm, 8u);
   // ---- reverse A9: plasticity (Eq.11), then the frame transport
   if (P.plasticity) {
     const float Y = c.sigy * c.l0;
@@ -164,7 +164,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.x[0] += shfl3(send, tp.pl);
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 16u);
   // ---- reverse A8 commit
   f3 velbar[VPL];
   GraspAcc ga;
@@ -186,7 +186,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     A.x[0] += shfl3(send, tp.pl);
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 32u);
   // ---- reverse A7 rigid coupling
   f3 ybar[VPL];
 #pragma unroll
@@ -198,7 +198,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     }
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 64u);
   // ---- reverse A6 friction + reconciliation.  velbar is now the adjoint of v^3.
   if (P.self_contact && R.ncand > 0) {
     for (int p = tp.lane; p < R.ncand; p += 32) sm.dpbar[p] = 0.0f;
@@ -236,7 +236,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     Sb[k] = 0.0f;
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 128u);
   // ---- reverse A5: iterations backwards; each Eq.10 update is undone from its stored multiplier
   f3 epred[VPL];   // the forward's predicted edge vectors, by the forward's expression (positions re-read: they are not held across the reverse of A9..A6)
   {
@@ -332,7 +332,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     xpb[0] += shfl3(send, tp.pl);
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 256u);
   // ---- reverse A4 predict, A3 velocity
   LaneState<VPL> s0b;
   load_state<VPL>(s0blk, tp.base, P.NS, s0b);
@@ -355,7 +355,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   }
   ga.flush(sm);
 
-  phase_sync(sm);
+  phase_sync(sm, 512u);
   // ---- reverse A2 forces: bending elements (and the stretch force in ENERGY mode) -> old edge geometry
   {
     EdgeCache<VPL> eb0;
@@ -410,7 +410,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   }
 
   G.gm[GM_RC] += (double)gm_rc; G.gm[GM_SIGY] += (double)gm_sigy; G.gm[GM_GAMMA] += (double)gm_gamma;
-  phase_sync(sm);
+  phase_sync(sm, 1024u);
   // ---- reverse A1: pose adjoints -> action adjoints (lane g owns gripper g)
   if (P.G > 0) {
     __syncwarp();

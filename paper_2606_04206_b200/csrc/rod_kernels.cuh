@@ -8,8 +8,12 @@ namespace dlo {
 // warps (= envs) per CTA: the CTA's warps walk the kernel in lockstep (phase_sync), so more warps per CTA share each
 // instruction-cache fill.  Forward: 2 CTAs of 4..8 warps per SM at <= 128 registers (the register file is split four ways: 16 K registers per scheduler, so more than 3 warps on a scheduler means <= 128 registers each); the host picks the count that fills whole waves; adjoint: 1 CTA of 8 warps at 255.
 // (upper bounds: the host lowers them when the per-warp shared memory of a large rope would not fit)
+#ifndef DLO_FWD_WARPS
 #define DLO_FWD_WARPS 8
+#endif
+#ifndef DLO_ADJ_WARPS
 #define DLO_ADJ_WARPS 8
+#endif
 
 // ---------------------------------------------------------------------------------------------------------
 // host-side helpers shared with the launcher

@@ -11,6 +11,7 @@ struct WarpSmem {
   unsigned short* cand;
   unsigned short* hot;   // near pairs of the last full filter (in pair order), kept across substeps
   float* base;        // the warp's shared-memory block (non-inlined helpers rebuild the view from this one pointer)
+  unsigned phase_mask;   // KParams::phase_mask
   int sync_threads;   // > 0: warps of the CTA walk the phases in lockstep (named barrier over this many threads)
   int NP;   // row stride of the per-vertex arrays: 33*VPL (32*VPL vertices + pad words, see vpos)
   __device__ __forceinline__ void init(const KParams& P, float* base, int np) {
@@ -21,13 +22,14 @@ struct WarpSmem {
     NP = np;
     this->base = base;
     sync_threads = 0;
+    phase_mask = P.phase_mask;
   }
 };
 
 // Phase barrier of the big kernels.  All warps of a CTA run the same long instruction stream on different envs; kept
 // in step, one instruction-cache fill serves all of them.  Must only be called from CTA-uniform control flow.
-__device__ __forceinline__ void phase_sync(const WarpSmem& sm) {
-  if (sm.sync_threads > 0) asm volatile("bar.sync 1, %0;" ::"r"(sm.sync_threads) : "memory");
+__device__ __forceinline__ void phase_sync(const WarpSmem& sm, unsigned site_bit = 1u) {
+  if (sm.sync_threads > 0 && (sm.phase_mask & site_bit)) asm volatile("bar.sync 1, %0;" ::"r"(sm.sync_threads) : "memory");
 }
 
 // Phase barrier that also ORs a per-thread flag over the CTA (bar.red): the warps decide together, at no extra cost
@@ -140,7 +142,7 @@ __device__ __forceinline__ Pose<float> read_pose(const float* o, int which) {
 }
 // target of a grasped vertex at the end of the substep: p1 + R1 q  (L103 kinematic flag, R-19), as a two-float sum hi + lo
 __device__ __forceinline__ f3 grasp_target(const KParams& P, const WarpSmem& sm, int code, f3& lo) {
-  const int slot = code - KIN_GRASP0, g = slot / P.M;
+  const int slot = code - KIN_GRASP0, g = (slot >= P.M) + (slot >= 2 * P.M) + (slot >= 3 * P.M);   // slot / M for G <= 4, without the division
   const float* o = sm.pose + g * POSE_STRIDE;
   const float* q = sm.q + 3 * slot;
   Pose<float> g1 = read_pose(o, 1);
@@ -507,10 +509,10 @@ __device__ __forceinline__ void project_edge_pre(const f3& e, float l0, float at
 // edge); on exit it holds that of the new positions.  ap/ac: this step's a_{t-1}, a_t of gripper `lane` (lane<G).
 // the barriers of substep() for a warp that skips the recompute (it must still take part in them, votes included)
 __device__ __forceinline__ void substep_idle_syncs(const KParams& P, const WarpSmem& sm) {
-  phase_sync(sm);
+  phase_sync(sm, 1u);
   if ((P.vote_mode & 1) && phase_vote(sm, false) && (P.vote_mode & 2)) phase_vote(sm, false);
-  phase_sync(sm);
-  phase_sync(sm);
+  phase_sync(sm, 2u);
+  phase_sync(sm, 4u);
 }
 // MODE 0: plain forward.  MODE 1 (REC): recompute inside the adjoint kernel (contact corrections -> acc_tape).
 // MODE 2 (TAPE): replay of a segment.  In both, the Eq.10 multipliers go to the tape rows `lam_rows` [N_C][NS].
@@ -523,7 +525,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // -- A1 bodies
   if (P.G > 0) publish_poses(P, env, tp.lane, ap, ac, sub, sm.pose, MODE != 1 && sub > 0);
 
-  phase_sync(sm);
+  phase_sync(sm, 1u);
   // -- A2 forces: gravity, stretch (mode ENERGY, Eq.2-3), bending (Eq.4-7)
   f3 f[VPL];
 #pragma unroll
@@ -833,7 +835,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     __syncwarp();
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 2u);
   // -- A7 rigid soft coupling at y = x^p + dx
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
@@ -865,7 +867,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     else if (tp.vvalid[k]) s.v[k] = zero3<float>();
   }
 
-  phase_sync(sm);
+  phase_sync(sm, 4u);
   // -- A9 frames: time-parallel transport (R-4), then plasticity (Eq.11)
   edge_refresh<VPL>(tp, s, ec);
 #pragma unroll

@@ -32,6 +32,7 @@ enum { PRIM_NP = 10, PRIM_SM_STRIDE = 20, PRIM_BC = 16, PRIM_BR = 19 };
 struct KParams {
   int B, N, E, NS /* padded row length */, ring, odd_ring, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip;
   int G, M, K, cand_cap, hot_cap;
+  unsigned phase_mask;   // which of the lockstep phase barriers are taken (tuning: DLO_PHASES; bit = site)
   int checks;            // DLO_CHECKS=1: guard words behind every per-warp shared-memory region, verified when a kernel ends
   int n_guard, sm_guard[24];   // their positions (float offsets from the warp's base)
   int t_base;            // frame index of the rollout's first step: step t of the launch uses actions[t_base + t - 1], actions[t_base + t]
