@@ -168,6 +168,38 @@ dlo_status dlo_set_kernel_timing(dlo_sim* sim, int32_t on);
 dlo_status dlo_get_kernel_timing(dlo_sim* sim, int32_t kernel_class, int32_t* n_launches, double* total_ms, int64_t* env_steps);
 dlo_status dlo_measure_fp32_peak(void* cuda_stream, double* tflops, double* elapsed_ms, int32_t* n_sm);
 
+/* Forward rollout WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  No handle: one call = dlo_create + scene + dlo_set_state + dlo_rollout_forward
+ * (stride 0) + dlo_get_state of a problem small enough that everything the handle would allocate (packed material,
+ * kinematic codes, grasp-local coordinates, the working state, per-env flags) fits a device array of
+ * DLO_STATIC_SCRATCH_BYTES that is part of the library image (every GPU that loads the library holds it until exit).
+ * dlo_static_scratch_bytes(cfg) = the bytes a config needs (0 for an invalid config); a config that needs more is refused
+ * with DLO_ERR_UNSUPPORTED (4 MiB holds e.g. 1024 envs x 64 vertices or 256 x 256).  Same kernels and results as the
+ * handle path.  The call issues a memset, five kernels and at most one device-to-device copy on `cuda_stream` and
+ * returns without synchronising; it calls no cudaMalloc / cudaFree / allocating routine.  (The very first call on a device
+ * resolves the array's address with cudaGetSymbolAddress: make that one outside graph capture.)
+ *   cfg, mat: as dlo_create (mat: dev pointers, each [B]).  scene: may be NULL when there are no pins, primitives or
+ *   grippers; otherwise the arguments of dlo_set_pins / dlo_set_primitives / dlo_set_grippers / dlo_set_actions (actions
+ *   [>= horizon][B][G][6]); pointers that the config does not need are ignored.  x0, v0 dev [B][3][N]; kappa_bar0 dev
+ *   [B][2][N] or NULL.  Outputs (dev, caller-owned, each may be NULL): x_T, v_T [B][3][N]; env_flags [B] int32, 0 = fine,
+ *   else the per-env bits dlo_check_numerics counts (1 non-finite, 2 candidate overflow, 4 guard).
+ * The scratch array is SHARED by all calls and keeps the last call's contents: the part a call uses is cleared when the call
+ * starts.  Calls whose work overlaps on the GPU (two streams without an event between them, two host threads) race on it;
+ * calls on one stream, or ordered by events, are safe. */
+#define DLO_STATIC_SCRATCH_BYTES (4u << 20)
+typedef struct {
+  const uint8_t* pinned;       /* dev [B][N] or NULL */
+  const int32_t* prim_types;   /* host [K] */
+  const float* prim_params;    /* dev [B][K][10] */
+  const float *init_pose, *finger_geom;   /* dev [B][G][6], [B][G][4] */
+  const int32_t* grasp_verts;  /* dev [B][G][M] */
+  const float* actions;        /* dev [H][B][G][6] */
+} dlo_scene;
+size_t dlo_static_scratch_bytes(const dlo_config* cfg);
+dlo_status dlo_rollout_forward_static(const dlo_config* cfg, const dlo_material* mat, const dlo_scene* scene, const float* x0,
+                                      const float* v0, const float* kappa_bar0, int32_t horizon, float* x_T, float* v_T,
+                                      int32_t* env_flags, void* cuda_stream);
+
 /* Number of kernel launches issued on this handle since create (bench.py's gpu_launches). */
 int64_t dlo_launch_count(const dlo_sim* sim);
 

@@ -6,4 +6,4 @@ importing works anywhere (so the build check can run without a GPU) but every co
 from .binding import (DloConfig, DloMaterial, DloSim, DloError, lib, dlo_create, dlo_destroy, dlo_set_pins,  # noqa: F401
                       dlo_set_primitives, dlo_set_grippers, dlo_set_state, dlo_restore_state, dlo_set_actions,
                       dlo_rollout_forward, dlo_get_state, dlo_get_position_residual, dlo_backward, dlo_get_state_adjoint, dlo_rollout_forward_host, dlo_backward_host, dlo_check_numerics,
-                      dlo_set_kernel_timing, dlo_get_kernel_timing, dlo_measure_fp32_peak, dlo_scratch_bytes, dlo_launch_count, dlo_last_error, dlo_version, EXPORTS)
+                      dlo_set_kernel_timing, dlo_get_kernel_timing, dlo_measure_fp32_peak, dlo_scratch_bytes, dlo_static_scratch_bytes, dlo_rollout_forward_static, make_config, STATIC_SCRATCH_BYTES, dlo_launch_count, dlo_last_error, dlo_version, EXPORTS)

@@ -15,8 +15,9 @@ STATUS_CALLS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_primitives
                 "dlo_restore_state", "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_get_position_residual",
                 "dlo_backward",
                 "dlo_get_state_adjoint", "dlo_rollout_forward_host", "dlo_backward_host", "dlo_check_numerics",
-                "dlo_set_kernel_timing", "dlo_get_kernel_timing", "dlo_measure_fp32_peak")
-EXPORTS = STATUS_CALLS + ("dlo_scratch_bytes", "dlo_launch_count", "dlo_last_error", "dlo_version")
+                "dlo_set_kernel_timing", "dlo_get_kernel_timing", "dlo_measure_fp32_peak", "dlo_rollout_forward_static")
+EXPORTS = STATUS_CALLS + ("dlo_scratch_bytes", "dlo_static_scratch_bytes", "dlo_launch_count", "dlo_last_error", "dlo_version")
+STATIC_SCRATCH_BYTES = 4 << 20   # DLO_STATIC_SCRATCH_BYTES of include/dlo.h
 MATERIAL_KEYS = ("mass_per_vertex", "rest_edge_len", "stretch", "bend_stiffness", "damping", "yield_curv",
                  "creep_rate", "mu_rigid", "mu_self")
 STATUS = {0: "DLO_OK", -1: "DLO_ERR_INVALID_ARG", -2: "DLO_ERR_BAD_STATE", -3: "DLO_ERR_CUDA", -4: "DLO_ERR_OOM",
@@ -33,6 +34,10 @@ class DloConfig(C.Structure):
 
 class DloMaterial(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in MATERIAL_KEYS]
+
+
+class DloScene(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("pinned", "prim_types", "prim_params", "init_pose", "finger_geom", "grasp_verts", "actions")]
 
 
 class DloError(RuntimeError):
@@ -55,6 +60,7 @@ def lib():
         L.dlo_last_error.restype = C.c_char_p
         L.dlo_version.restype = C.c_char_p
         L.dlo_scratch_bytes.restype = C.c_size_t
+        L.dlo_static_scratch_bytes.restype = C.c_size_t
         L.dlo_launch_count.restype = C.c_int64
         L.dlo_launch_count.argtypes = [C.c_void_p]
         for name in STATUS_CALLS:
@@ -187,6 +193,29 @@ def dlo_measure_fp32_peak(stream=0):
 
 def dlo_scratch_bytes(cfg: DloConfig, horizon, checkpoint_stride):
     return int(lib().dlo_scratch_bytes(C.byref(cfg), C.c_int32(horizon), C.c_int32(checkpoint_stride)))
+
+
+def dlo_static_scratch_bytes(cfg: DloConfig):
+    return int(lib().dlo_static_scratch_bytes(C.byref(cfg)))
+
+
+def dlo_rollout_forward_static(cfg: DloConfig, material: dict, scene: dict, x0, v0, kappa_bar0, horizon, x_T=None, v_T=None,
+                               env_flags=None, stream=0):
+    """The forward rollout without any allocation in the library (scratch in a static device array; include/dlo.h).  `scene`:
+    dict with any of pinned, prim_types (host int32 array), prim_params, init_pose, finger_geom, grasp_verts, actions."""
+    m = DloMaterial()
+    for k in MATERIAL_KEYS:
+        setattr(m, k, material[k].data_ptr())
+    sc = DloScene()
+    keep = None
+    for k, _ in DloScene._fields_:
+        v = (scene or {}).get(k)
+        if k == "prim_types" and v is not None:
+            keep = v = np.ascontiguousarray(v, dtype=np.int32)
+        setattr(sc, k, _p(v).value)
+    _chk(lib().dlo_rollout_forward_static(C.byref(cfg), C.byref(m), C.byref(sc), _p(x0), _p(v0), _p(kappa_bar0), C.c_int32(horizon),
+                                          _p(x_T), _p(v_T), _p(env_flags), C.c_void_p(stream)))
+    del keep
 
 
 def dlo_launch_count(h):

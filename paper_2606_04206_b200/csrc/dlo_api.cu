@@ -603,3 +603,4 @@ dlo_status dlo_check_numerics(dlo_sim* s, int32_t* n_bad) {
 
 #include "dlo_api_backward.inl"
 #include "dlo_bench.inl"
+#include "dlo_noalloc.inl"
