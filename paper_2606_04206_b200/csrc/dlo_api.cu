@@ -344,6 +344,8 @@ dlo_status dlo_set_primitives(dlo_sim* s, const int32_t* types, const float* par
     if (types[k] < 0 || types[k] > 3) return fail(DLO_ERR_INVALID_ARG, "unknown primitive type");
     s->P.prim_type[k] = types[k];
   }
+  s->P.prim_pack = 0u;
+  for (int k = 0; k < s->P.K; ++k) s->P.prim_pack |= (unsigned)types[k] << (2 * k);
   CU(cudaMemcpyAsync(s->prim, params, (size_t)s->P.B * s->P.K * PRIM_NP * sizeof(float), cudaMemcpyDeviceToDevice, s->stream));
   s->have_prims = true;
   return DLO_OK;

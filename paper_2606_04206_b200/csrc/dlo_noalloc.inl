@@ -81,6 +81,7 @@ dlo_status dlo_rollout_forward_static(const dlo_config* cfg, const dlo_material*
   for (int k = 0; k < P.K; ++k) {
     if (scene->prim_types[k] < 0 || scene->prim_types[k] > 3) return fail(DLO_ERR_INVALID_ARG, "unknown primitive type");
     P.prim_type[k] = scene->prim_types[k];
+    P.prim_pack |= (unsigned)scene->prim_types[k] << (2 * k);
   }
   const StaticLayout L = static_layout(P);
   if (L.total > (size_t)DLO_STATIC_SCRATCH_BYTES)

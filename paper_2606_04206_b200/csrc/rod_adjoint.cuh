@@ -76,9 +76,9 @@ struct GraspAcc {
 };
 
 // one rigid body (primitive b < K, else finger (b-K)) evaluated at y: phi, n, body velocity
-__device__ __forceinline__ bool body_eval(const KParams& P, const WarpSmem& sm, int b, const f3& y, float& phi, f3& n, f3& vb) {
+__device__ __forceinline__ bool body_eval(const CoupleConst& P, const WarpSmem& sm, int b, const f3& y, float& phi, f3& n, f3& vb) {
   vb = zero3<float>();
-  if (b < P.K) return sdf_eval_pre<float>(P.prim_type[b], sm.prim + b * PRIM_SM_STRIDE, y, phi, n);
+  if (b < P.K) return sdf_eval_pre<float>((int)((P.types >> (2 * b)) & 3u), sm.prim + b * PRIM_SM_STRIDE, y, phi, n);
   const int g = (b - P.K) >> 1, fk = (b - P.K) & 1;
   const float* o = sm.pose + g * POSE_STRIDE;
   const float* A = o + (fk ? POSE_FA1 : POSE_FA0);
@@ -92,10 +92,10 @@ __device__ __forceinline__ bool body_eval(const KParams& P, const WarpSmem& sm, 
 // reverse of A7 for one free vertex: `active` = bodies that responded (forward order = bit order), v3 = velocity
 // before the coupling.  velbar: in = adjoint of v4, out = adjoint of v3.  ybar += adjoint of y.
 struct CoupleAdj { f3 velbar, ybar; };
-__device__ __noinline__ CoupleAdj rigid_coupling_adj(const KParams& P, float* smbase, int np, int env, unsigned active, f3 y, f3 v3, float mu_r,
+__device__ __noinline__ CoupleAdj rigid_coupling_adj(const KParams& __restrict__ KP, const CoupleConst P, float* smbase, int np, int env, unsigned active, f3 y, f3 v3, float mu_r,
                                                      f3 velbar) {
   WarpSmem sm;
-  sm.init(P, smbase, np);
+  sm.init(KP, smbase, np);
   f3 ybar = zero3<float>();
   unsigned m = active;
   while (m) {
@@ -116,7 +116,7 @@ __device__ __noinline__ CoupleAdj rigid_coupling_adj(const KParams& P, float* sm
     const float dbar = rigid_response_adj<float>(v, vb, n, P.r - phi, P.inv_eps, P.e_rest, mu_r, velbar, vbar, vbbar, nbar);
     velbar = vbar;
     const float phibar = -dbar;
-    if (b < P.K) sdf_pre_adj<float>(P.prim_type[b], sm.prim + b * PRIM_SM_STRIDE, y, phibar, nbar, ybar);
+    if (b < P.K) sdf_pre_adj<float>((int)((P.types >> (2 * b)) & 3u), sm.prim + b * PRIM_SM_STRIDE, y, phibar, nbar, ybar);
     else {
       const int g = (b - P.K) >> 1, fk = (b - P.K) & 1;
       const float* o = sm.pose + g * POSE_STRIDE;
@@ -126,7 +126,7 @@ __device__ __noinline__ CoupleAdj rigid_coupling_adj(const KParams& P, float* sm
       sdf_capsule_adj<float>(mk3<float>(A[0], A[1], A[2]), mk3<float>(Bp[0], Bp[1], Bp[2]), y, phibar, nbar, ybar, Abar, Bbar);
       PoseBar<float> b0, b1;
       pose_bar_zero(b0); pose_bar_zero(b1);
-      const float* fg = P.finger + ((size_t)env * P.G + g) * 4;
+      const float* fg = KP.finger + ((size_t)env * P.G + g) * 4;
       const float sx = (fk ? -0.5f : 0.5f) * fg[0];
       rigid_point_adj<float>(mk3<float>(sx, 0.f, 0.f), Abar, b1);
       rigid_point_adj<float>(mk3<float>(sx, 0.f, fg[1]), Bbar, b1);
@@ -161,7 +161,7 @@ template <int VPL> __device__ __forceinline__ void cand_verts(const WarpSmem& sm
 
 // reverse of one Eq.13 Jacobi pass: positions y (before the pass) in sm.ys, adjoint of the post-pass corrections
 // in sm.vbar, adjoint of D_p in sm.dpbar; position adjoints are summed into sm.ybar
-template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& P, int lane, float* smbase, int ncand) {
+template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& __restrict__ P, int lane, float* smbase, int ncand) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
@@ -188,7 +188,7 @@ template <int VPL> __device__ __noinline__ void contact_pass_adj(const KParams& 
 
 // reverse of the friction pass: y in sm.ys, v^2 in sm.vs, adjoint of v^3 in sm.vbar; writes sm.dpbar, sums
 // position adjoints into sm.ybar and velocity adjoints into sm.acc
-template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams& P, int lane, float* smbase, int ncand, float mu_s) {
+template <int VPL> __device__ __noinline__ void friction_pass_adj(const KParams& __restrict__ P, int lane, float* smbase, int ncand, float mu_s) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;

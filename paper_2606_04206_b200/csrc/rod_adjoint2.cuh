@@ -193,7 +193,7 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
   for (int k = 0; k < VPL; ++k) {
     ybar[k] = zero3<float>();
     if (c.kin[k] == KIN_FREE && R.active[k]) {
-      const CoupleAdj ca = rigid_coupling_adj(P, sm.base, sm.NP, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k]);
+      const CoupleAdj ca = rigid_coupling_adj(P, couple_const(P), sm.base, sm.NP, env, R.active[k], R.xp[k] + R.dx[k], R.v3[k], c.mu_r, velbar[k]);
       velbar[k] = ca.velbar; ybar[k] = ca.ybar;
     }
   }
@@ -259,9 +259,13 @@ __device__ __forceinline__ void substep_reverse(const KParams& P, const Topo<VPL
     const float wsum = c.w[k] + wfar[k];
     idn[k] = (P.stretch_mode == 1 && on && wsum > 0.0f) ? 1.0f / (wsum + atil) : 0.0f;
   }
+  float lam_next[VPL];   // multipliers one iteration ahead: the tape read of iteration it - 1 is in flight while iteration it is reversed
+  load_row<VPL>(s0blk + (size_t)(TAPE_LAM + (P.N_C > 0 ? P.N_C - 1 : 0)) * P.NS, tp.base, P.NS, lam_next);
   for (int it = P.N_C - 1; it >= 0; --it) {
     float lamv[VPL];   // multipliers of this iteration, one per owned edge (the odd ring's closing edge sits in its idle red slot)
-    load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it) * P.NS, tp.base, P.NS, lamv);
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) lamv[k] = lam_next[k];
+    if (it > 0) load_row<VPL>(s0blk + (size_t)(TAPE_LAM + it - 1) * P.NS, tp.base, P.NS, lam_next);
     if (P.self_contact && ((R.jac_mask >> it) & 1u)) {
 #pragma unroll
       for (int k = 0; k < VPL; ++k) {

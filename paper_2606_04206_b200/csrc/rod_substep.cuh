@@ -213,10 +213,13 @@ __device__ __forceinline__ float pair_dist2(const float* ys, int NP, int pa, int
 // for bit); it is not the oracle's lexicographic order (only the fp32 summation order of the Jacobi pass depends
 // on it).  mid = (midpoint, half length, w) at the positions the superset was built at.
 template <int VPL>
-__device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* smbase, float slack, float bx, float by, float bz, float br) {
+__device__ __noinline__ int build_pair_list(const KParams& __restrict__ P, int lane, float* smbase, float slack, float bx, float by, float bz, float br) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int E = P.E, NP = sm.NP, nb = (E + VPL - 1) / VPL;
+  // P is read through a reference here (a generic load per access, repeated in every loop iteration because of the stores
+  // to shared memory in between): the fields the loops use are taken once
+  const int self_skip = P.self_skip, ring = P.ring, cand_cap = P.cand_cap;
   const float lim = 4.0f * P.r + slack;   // 2 (r_a + r_b) + slack
   constexpr int PP = VPL * VPL, NPER = PP <= 32 ? 32 / PP : 1, ITER = (PP + 31) / 32;
   unsigned short* surv = sm.cand + P.cand_cap;
@@ -243,7 +246,7 @@ __device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* s
         for (int q = 0; q < NPER; ++q) { if (q == sub && mm) Bsel = __ffs(mm) - 1; mm &= mm - 1u; }
         const int ka = idx / VPL, kb = idx % VPL, a = A * VPL + ka, b = (int)Bsel * VPL + kb, d = b - a;
         bool hit = false;
-        if (Bsel != 0xffffffffu && idx < PP && sub < NPER && b < E && d >= P.self_skip && (!P.ring || E - d >= P.self_skip)) {
+        if (Bsel != 0xffffffffu && idx < PP && sub < NPER && b < E && d >= self_skip && (!ring || E - d >= self_skip)) {
           const int pa = vpos<VPL>(a), pb = vpos<VPL>(b);
           const float dx = sm.mid[pb] - sm.mid[pa], dy = sm.mid[NP + pb] - sm.mid[NP + pa], dz = sm.mid[2 * NP + pb] - sm.mid[2 * NP + pa];
           const float reach = sm.mid[3 * NP + pa] + sm.mid[3 * NP + pb] + lim;
@@ -252,7 +255,7 @@ __device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* s
         const unsigned m = __ballot_sync(DLO_FULL, hit);
         if (hit) {
           const int pos = nsurv + __popc(m & ((1u << lane) - 1u));
-          if (pos < P.cand_cap) surv[pos] = (unsigned short)((a << 8) | b);
+          if (pos < cand_cap) surv[pos] = (unsigned short)((a << 8) | b);
         }
         nsurv += __popc(m);
       }
@@ -270,7 +273,7 @@ __device__ __noinline__ int build_pair_list(const KParams& P, int lane, float* s
 // bound on dfar.  Too many near pairs for sm.hot: no near list (nhot = -1), dfar covers every pair.
 struct CandOut { int ncand, nhot; float dmin, dfar; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b); dfar: over the far ones
 template <int VPL>
-__device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, float* smbase, int nsurv, bool overflow) {
+__device__ __noinline__ CandOut filter_candidates(const KParams& __restrict__ P, int lane, float* smbase, int nsurv, bool overflow) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int N = P.N, NP = sm.NP;
@@ -313,7 +316,7 @@ __device__ __noinline__ CandOut filter_candidates(const KParams& P, int lane, fl
 
 // the near pairs measured again at x^p (in sm.ys): candidate list = those closer than 2(r_a+r_b), in pair order
 template <int VPL>
-__device__ __noinline__ CandOut filter_near(const KParams& P, int lane, float* smbase, int nhot) {
+__device__ __noinline__ CandOut filter_near(const KParams& __restrict__ P, int lane, float* smbase, int nhot) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int N = P.N, NP = sm.NP;
@@ -361,7 +364,7 @@ __device__ __forceinline__ void ordered_scatter4(unsigned hits, int lane, float*
 // A5(ii): one Jacobi pass of Eq.13 over the candidates at y (in sm.ys); corrections summed into sm.acc, D_p += d.
 // Returns true if any correction was applied.
 template <int VPL>
-__device__ __noinline__ bool contact_pass(const KParams& P, int lane, float* smbase, int ncand) {
+__device__ __noinline__ bool contact_pass(const KParams& __restrict__ P, int lane, float* smbase, int ncand) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
@@ -405,7 +408,7 @@ __device__ __noinline__ bool contact_pass(const KParams& P, int lane, float* smb
 
 // A6 self-contact friction (L410, R-16) for candidates with D_p > 0: velocities in sm.vs, positions in sm.ys
 template <int VPL>
-__device__ __noinline__ void friction_pass(const KParams& P, int lane, float* smbase, int ncand, float mu_s) {
+__device__ __noinline__ void friction_pass(const KParams& __restrict__ P, int lane, float* smbase, int ncand, float mu_s) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int NP = sm.NP, N = P.N;
@@ -454,7 +457,20 @@ __device__ __noinline__ void friction_pass(const KParams& P, int lane, float* sm
 // Not inlined on purpose: it is called once per vertex slot and is the largest single piece of straight-line code
 // (four SDF types + fingers); one copy keeps the kernel inside the instruction cache.
 struct CoupleOut { f3 v; unsigned active; };
-__device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* __restrict__ prim_sm, const float* __restrict__ pose_sm,
+// the scalars of KParams that A7 needs, passed by value: inside a non-inlined function a field of the kernel's parameter
+// block is a generic load through a pointer, in the kernel it is a constant-bank operand
+struct CoupleConst {
+  int K, G;
+  float r, inv_eps, log_thresh_lo, f_thresh, e_rest, inv_h;
+  unsigned types;   // prim_type[k] in bits 2k, 2k+1
+};
+__device__ __forceinline__ CoupleConst couple_const(const KParams& P) {
+  CoupleConst q;
+  q.K = P.K; q.G = P.G; q.r = P.r; q.inv_eps = P.inv_eps; q.log_thresh_lo = P.log_thresh_lo; q.f_thresh = P.f_thresh; q.e_rest = P.e_rest; q.inv_h = P.inv_h;
+  q.types = P.prim_pack;
+  return q;
+}
+__device__ __noinline__ CoupleOut rigid_coupling(const CoupleConst P, const float* __restrict__ prim_sm, const float* __restrict__ pose_sm,
                                                  f3 y, f3 v, float mu_r) {
   unsigned active = 0u;
   // a body whose bounding sphere is farther than reach = r + eps_s |ln f_thresh| cannot pass the f > f_thresh test
@@ -468,7 +484,7 @@ __device__ __noinline__ CoupleOut rigid_coupling(const KParams& P, const float* 
     }
     float phi;
     f3 n;
-    if (!sdf_eval_pre<float>(P.prim_type[k], pk, y, phi, n)) continue;
+    if (!sdf_eval_pre<float>((int)((P.types >> (2 * k)) & 3u), pk, y, phi, n)) continue;
     if ((P.r - phi) * P.inv_eps < P.log_thresh_lo) continue;
     if (rigid_response<float>(v, zero3<float>(), n, P.r - phi, P.inv_eps, P.f_thresh, P.e_rest, mu_r)) active |= 1u << k;
   }
@@ -842,7 +858,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     R.v3[k] = vel[k];
     R.active[k] = 0u;
     if (c.kin[k] == KIN_FREE && (P.K > 0 || P.G > 0)) {
-      const CoupleOut co = rigid_coupling(P, sm.prim, sm.pose, XP(k) + R.dx[k], vel[k], c.mu_r);
+      const CoupleOut co = rigid_coupling(couple_const(P), sm.prim, sm.pose, XP(k) + R.dx[k], vel[k], c.mu_r);
       vel[k] = co.v; R.active[k] = co.active;
     }
     R.v4[k] = vel[k];

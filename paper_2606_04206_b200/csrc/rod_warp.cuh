@@ -41,6 +41,7 @@ struct KParams {
   float near_dist;       // pairs closer than this at a full filter go to the near list (measured every substep)
   float list_margin;     // the self-contact pair list stays valid while no vertex has moved further than this since it was built
   int prim_type[16];
+  unsigned prim_pack;    // prim_type[k] in bits 2k, 2k+1 (what the non-inlined A7 takes by value)
   const float* mat;      // [B][MAT_N]
   const uint8_t* kin;    // [B][NS]
   const float* qloc;     // [B][G*M][3]
