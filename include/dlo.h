@@ -91,6 +91,14 @@ dlo_status dlo_destroy(dlo_sim* sim);
  *   fingers from p + R(+-gap/2,0,0) to p + R(+-gap/2,0,length)); grasp_verts dev [B][G][M] int32, -1 = none:
  *   vertices carried rigidly by the gripper (kinematic, L103). */
 dlo_status dlo_set_pins(dlo_sim* sim, const uint8_t* pinned);
+/* Several DLOs in one env (PAPER.md L145 Separation, L155 Letter Art: Eq.13 acts between different ropes, L406).  The ropes
+ * lie back to back in the env's vertex array; cut: dev [B][N] uint8, non-zero at vertex j = the edge (j, j+1) does not exist
+ * (the last entry is ignored).  An absent edge carries no stretch force / Eq.10 constraint, no frame (its d1 column stays 0)
+ * and is no self-contact segment; the vertices next to it are rope ends (no bending element, no rest curvature); the frames
+ * of A0 start afresh at the first edge of every rope.  All ropes of an env share its material, radius and rest edge length;
+ * every pair of existing edges at index distance >= self_skip is a contact pair, within a rope or across ropes.  Call
+ * before dlo_set_state.  DLO_ERR_UNSUPPORTED for the ring topology (one closed band per env) or self_skip != 2. */
+dlo_status dlo_set_cuts(dlo_sim* sim, const uint8_t* cut);
 dlo_status dlo_set_primitives(dlo_sim* sim, const int32_t* types, const float* params);
 dlo_status dlo_set_grippers(dlo_sim* sim, const float* init_pose, const float* finger_geom, const int32_t* grasp_verts);
 

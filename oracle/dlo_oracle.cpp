@@ -30,6 +30,7 @@ struct EnvD {
   std::vector<State<double>> ckpt;       // checkpoint g = state after g*stride steps
   std::vector<State<double>> rec;        // optional per-step record (rec[t] = state after t steps)
   double margin[MG_COUNT];               // diagnostics: closest approach to each branch threshold during the last rollout
+  std::vector<uint8_t> cut;              // [N] absent edges of a multi-DLO scene (empty: one rope)
 };
 
 struct oracle_sim {
@@ -43,6 +44,7 @@ struct oracle_sim {
 
 static Config to_config(const oracle_config& o) {
   Config c;
+  c.cut = nullptr;
   c.N = o.n_verts; c.topology = o.topology; c.n_sub = o.n_substeps; c.N_C = o.n_proj_iters;
   c.stretch_mode = o.stretch_mode; c.plasticity = o.enable_plasticity; c.self_contact = o.enable_self_contact;
   c.self_skip = o.self_skip; c.G = o.n_grippers; c.n_grasp_max = o.n_grasp_max; c.K = o.n_primitives;
@@ -52,6 +54,8 @@ static Config to_config(const oracle_config& o) {
   return c;
 }
 
+// the env's own view of the shared config (its cuts)
+static Config env_config(const oracle_sim* h, int b);
 static void recompute_kin(const Config& c, Scene& sc, const std::vector<uint8_t>& pinned) {
   sc.kin.assign(c.N, KIN_FREE); sc.grasp_g.assign(c.N, -1); sc.grasp_k.assign(c.N, -1);
   for (int i = 0; i < c.N; ++i) if (!pinned.empty() && pinned[i]) sc.kin[i] = KIN_PINNED;
@@ -61,6 +65,12 @@ static void recompute_kin(const Config& c, Scene& sc, const std::vector<uint8_t>
       int v = sc.grasp_vert[g * c.n_grasp_max + k];
       if (v >= 0 && v < c.N) { sc.kin[v] = KIN_GRASPED; sc.grasp_g[v] = g; sc.grasp_k[v] = k; }
     }
+}
+
+static Config env_config(const oracle_sim* h, int b) {
+  Config c = h->c;
+  c.cut = h->env[b].cut.empty() ? nullptr : h->env[b].cut.data();
+  return c;
 }
 
 template <class T> static State<T> lift(const State<double>& s) {
@@ -119,11 +129,19 @@ void oracle_set_grippers(oracle_sim* h, const double* init_pose /* [B][G][6] */,
   }
 }
 
-// A0: frames, rest curvature, grasp-local coordinates.  Call after pins / grippers are set.
+// Multi-DLO scenes: cut[b][j] != 0 removes edge (j, j+1) of env b (rod_step.hpp, Config::cut).  Open topology only.
+int32_t oracle_set_cuts(oracle_sim* h, const uint8_t* cut /* [B][N] */) {
+  if (h->c.topology != TOPO_OPEN) return -1;
+  for (int b = 0; b < h->B; ++b) h->env[b].cut.assign(cut + (size_t)b * h->c.N, cut + (size_t)(b + 1) * h->c.N);
+  return 0;
+}
+
+// A0: frames, rest curvature, grasp-local coordinates.  Call after pins / grippers / cuts are set.
 void oracle_set_state(oracle_sim* h, const double* x0, const double* v0, const double* kbar0 /* or NULL */) {
-  const Config& c = h->c; const int N = c.N, E = c.E();
+  const int N = h->c.N, E = h->c.E();
 #pragma omp parallel for schedule(dynamic)
   for (int b = 0; b < h->B; ++b) {
+    const Config c = env_config(h, b);
     EnvD& e = h->env[b];
     State<double>& s = e.s0;
     s.x.resize(N); s.v.resize(N); s.k1.assign(N, 0.0); s.k2.assign(N, 0.0);
@@ -209,12 +227,12 @@ static const double* action_ptr(const oracle_sim* h, int b, int t) {   // a_t, t
 // forward rollout from the state set by oracle_set_state.  stride>0: keep checkpoint every `stride` steps.
 // record != 0: additionally keep the state after every step (for the pins that look at trajectories).
 int32_t oracle_rollout_forward(oracle_sim* h, int32_t horizon, int32_t stride, int32_t record) {
-  const Config& c = h->c;
-  if (c.G > 0 && h->t_start + horizon > h->H_actions) return -1;
+  if (h->c.G > 0 && h->t_start + horizon > h->H_actions) return -1;
   const int ts = h->t_start;
   h->stride = stride; h->record = record; h->H_done = horizon;
 #pragma omp parallel for schedule(dynamic)
   for (int b = 0; b < h->B; ++b) {
+    const Config c = env_config(h, b);
     EnvD& e = h->env[b];
     Work<double> w;
     e.cur = e.s0; e.ckpt.clear(); e.rec.clear();
@@ -274,12 +292,13 @@ int32_t oracle_get_record(oracle_sim* h, int32_t t, double* x, double* v, double
 int32_t oracle_backward(oracle_sim* h, const double* gxT, const double* gvT, double* g_actions /* [H][B][G][6] */,
                         double* g_x0, double* g_v0, double* g_d10 /* [B][3][N], extra */, double* g_kbar0 /* [B][2][N], extra */,
                         double* g_material /* [B][5] */) {
-  const Config& c = h->c; const int N = c.N, E = c.E(), G = c.G, H = h->H_done, stride = h->stride;
+  const int N = h->c.N, E = h->c.E(), G = h->c.G, H = h->H_done, stride = h->stride;
   if (stride <= 0 || H <= 0) return -2;
   const int ts = h->t_start;   // frames are ts + t; g_actions is indexed by t (relative to the rollout's start)
   if (g_actions) std::memset(g_actions, 0, sizeof(double) * (size_t)H * h->B * G * 6);
 #pragma omp parallel for schedule(dynamic)
   for (int b = 0; b < h->B; ++b) {
+    const Config c = env_config(h, b);
     EnvD& e = h->env[b];
     Tape tape; current_tape() = &tape;
     Work<double> wd; Work<AD> wa;

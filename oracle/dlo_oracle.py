@@ -32,7 +32,7 @@ def lib():
         _lib.oracle_op_bend_energy.restype = _F
         _lib.oracle_op_stretch_energy.restype = _F
         for name in ("oracle_rollout_forward", "oracle_backward", "oracle_get_record", "oracle_num_threads",
-                     "oracle_op_self_contact", "oracle_op_sdf", "oracle_num_margins"):
+                     "oracle_op_self_contact", "oracle_op_sdf", "oracle_num_margins", "oracle_set_cuts"):
             getattr(_lib, name).restype = C.c_int32
     return _lib
 
@@ -78,6 +78,10 @@ class OracleSim:
         if problem.get("pins") is not None:
             pins = np.ascontiguousarray(problem["pins"][self.envs], dtype=np.uint8)
             L.oracle_set_pins(self.h, _ptr(pins))
+        if problem.get("cuts") is not None:      # several DLOs in one env: absent edges
+            cuts = np.ascontiguousarray(problem["cuts"][self.envs], dtype=np.uint8)
+            if L.oracle_set_cuts(self.h, _ptr(cuts)) != 0:
+                raise ValueError("cuts need the open topology")
         if self.K > 0:
             types = np.ascontiguousarray(problem["prim_types"], dtype=np.int32)
             L.oracle_set_primitives(self.h, _ptr(types), _ptr(_d(problem["prim_params"][self.envs])))

@@ -69,8 +69,14 @@ struct Config {
   int N, topology, n_sub, N_C, stretch_mode, plasticity, self_contact, self_skip, G, n_grasp_max, K;
   int kappa_bar_from_x0;
   double dt, g[3], r, eps_s, f_thresh, e_rest;
+  // Several DLOs in one env (P:L145 Separation, P:L155 Letter Art: Eq.13 acts between different ropes): the ropes
+  // are laid back to back in the vertex array of an OPEN topology and cut[j] != 0 says that edge j (j, j+1) does not
+  // exist.  Borrowed, [N], or null = one rope.  An absent edge carries no stretch / Eq.10 constraint, no frame and is no
+  // self-contact segment; a vertex next to it is a rope END (no bending, no rest curvature).
+  const uint8_t* cut;
   int E() const { return topology == TOPO_RING ? N : N - 1; }
 };
+inline bool edge_exists(const Config& c, int j) { return !(c.cut && c.cut[j]); }
 
 // constants of one environment (never differentiated)
 struct Scene {
@@ -97,7 +103,10 @@ template <class T> struct State {
 // vertex/edge index helpers (open: edge j joins j,j+1; ring: j,(j+1) mod N)
 inline int vnext(const Config& c, int i) { return (c.topology == TOPO_RING) ? (i + 1) % c.N : i + 1; }
 inline int vprev(const Config& c, int i) { return (c.topology == TOPO_RING) ? (i + c.N - 1) % c.N : i - 1; }
-inline bool interior(const Config& c, int i) { return c.topology == TOPO_RING || (i >= 1 && i <= c.N - 2); }
+inline bool interior(const Config& c, int i) {
+  if (c.topology == TOPO_RING) return true;
+  return i >= 1 && i <= c.N - 2 && edge_exists(c, i - 1) && edge_exists(c, i);
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // Rodrigues: R = exp([rho]x) (App. A step 1; series for |rho| < 1e-4)
@@ -147,10 +156,16 @@ inline void frames_init(const Config& c, const std::vector<Vec3<double>>& x, std
   for (int j = 0; j < E; ++j) { Vec3<double> e = x[vnext(c, j)] - x[j]; t[j] = (1.0 / norm(e)) * e; }
   d1.assign(E, zero3<double>());
   Vec3<double> zhat = mkv(0.0, 0.0, 1.0), yhat = mkv(0.0, 1.0, 0.0);
-  Vec3<double> ref = (norm(cross(t[0], zhat)) < 1e-6) ? yhat : zhat;
-  Vec3<double> u = ref - dot(ref, t[0]) * t[0];
-  d1[0] = (1.0 / norm(u)) * u;
-  for (int j = 1; j < E; ++j) d1[j] = ptransport(t[j - 1], t[j], d1[j - 1]);
+  bool first = true;                                  // the first edge of every rope starts a chain of its own
+  for (int j = 0; j < E; ++j) {
+    if (!edge_exists(c, j)) { first = true; continue; }   // absent edge: no frame (left at zero)
+    if (first) {
+      Vec3<double> ref = (norm(cross(t[j], zhat)) < 1e-6) ? yhat : zhat;
+      Vec3<double> u = ref - dot(ref, t[j]) * t[j];
+      d1[j] = (1.0 / norm(u)) * u;
+      first = false;
+    } else d1[j] = ptransport(t[j - 1], t[j], d1[j - 1]);
+  }
   double psiH = 0.0;
   if (c.topology == TOPO_RING) {
     Vec3<double> uu = ptransport(t[E - 1], t[0], d1[E - 1]);     // transported once around the loop
@@ -217,6 +232,7 @@ template <class T>
 T stretch_energy(const Config& c, const std::vector<Vec3<T>>& x, const T& ks, double l0) {
   T U = T(0.0);
   for (int j = 0; j < c.E(); ++j) {
+    if (!edge_exists(c, j)) continue;
     T eps = norm(x[vnext(c, j)] - x[j]) / l0 - 1.0;
     U += 0.5 * ks * eps * eps * l0;
   }
@@ -225,6 +241,7 @@ T stretch_energy(const Config& c, const std::vector<Vec3<T>>& x, const T& ks, do
 template <class T>
 void stretch_force(const Config& c, const std::vector<Vec3<T>>& x, const T& ks, double l0, std::vector<Vec3<T>>& f) {
   for (int j = 0; j < c.E(); ++j) {
+    if (!edge_exists(c, j)) continue;
     int jn = vnext(c, j);
     Vec3<T> e = x[jn] - x[j];
     T L = norm(e);
@@ -490,6 +507,7 @@ void substep(const Config& c, const Scene& sc, const Params<T>& pm, State<T>& st
     for (int a = 0; a < E; ++a)
       for (int b = a + 1; b < E; ++b) {
         if (cyclic_edge_distance(c, a, b) < c.self_skip) continue;
+        if (!edge_exists(c, a) || !edge_exists(c, b)) continue;
         Vec3<double> p1 = vval(w.xp[a]), q1 = vval(w.xp[vnext(c, a)]), p2 = vval(w.xp[b]), q2 = vval(w.xp[vnext(c, b)]);
         double t, u; closest_points(p1, q1, p2, q2, t, u);
         Vec3<double> dv = ((1.0 - t) * p1 + t * q1) - ((1.0 - u) * p2 + u * q2);
@@ -508,7 +526,7 @@ void substep(const Config& c, const Scene& sc, const Params<T>& pm, State<T>& st
       for (int colour = 0; colour < 3; ++colour) {
         for (int j = 0; j < E; ++j) {
           int col_j = (odd_ring && j == E - 1) ? 2 : (j & 1);
-          if (col_j != colour) continue;
+          if (col_j != colour || !edge_exists(c, j)) continue;
           int jn = vnext(c, j);
           project_edge(edge_vec(j), winv[j], winv[jn], l0, atil, w.S[j], w.dx[j], w.dx[jn]);
         }
@@ -595,7 +613,10 @@ void substep(const Config& c, const Scene& sc, const Params<T>& pm, State<T>& st
 
   // -- 8. commit (A8)
   w.t_old.assign(E, zero3<T>());
-  for (int j = 0; j < E; ++j) { Vec3<T> e = st.x[vnext(c, j)] - st.x[j]; w.t_old[j] = (T(1.0) / norm(e)) * e; }
+  for (int j = 0; j < E; ++j) {
+    if (!edge_exists(c, j)) continue;
+    Vec3<T> e = st.x[vnext(c, j)] - st.x[j]; w.t_old[j] = (T(1.0) / norm(e)) * e;
+  }
   for (int i = 0; i < N; ++i) {
     if (sc.kin[i] == KIN_FREE) { st.x[i] = st.x[i] + T(h) * vel[i]; st.v[i] = vel[i]; }
     else if (sc.kin[i] == KIN_PINNED) { st.v[i] = zero3<T>(); }
@@ -604,6 +625,7 @@ void substep(const Config& c, const Scene& sc, const Params<T>& pm, State<T>& st
 
   // -- 9. frames (time-parallel transport, reading B-4) + plasticity (Eq.11)
   for (int j = 0; j < E; ++j) {
+    if (!edge_exists(c, j)) continue;
     Vec3<T> e = st.x[vnext(c, j)] - st.x[j];
     Vec3<T> tn = (T(1.0) / norm(e)) * e;
     Vec3<T> d = ptransport(w.t_old[j], tn, st.d1[j]);

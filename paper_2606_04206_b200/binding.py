@@ -11,7 +11,7 @@ import numpy as np
 from . import build as _build
 
 _F = C.c_float
-STATUS_CALLS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_primitives", "dlo_set_grippers", "dlo_set_state",
+STATUS_CALLS = ("dlo_create", "dlo_destroy", "dlo_set_pins", "dlo_set_cuts", "dlo_set_primitives", "dlo_set_grippers", "dlo_set_state",
                 "dlo_restore_state", "dlo_set_actions", "dlo_rollout_forward", "dlo_get_state", "dlo_get_position_residual",
                 "dlo_backward",
                 "dlo_get_state_adjoint", "dlo_rollout_forward_host", "dlo_backward_host", "dlo_check_numerics",
@@ -113,6 +113,10 @@ def dlo_destroy(h):
 
 def dlo_set_pins(h, pinned):
     _chk(lib().dlo_set_pins(h, _p(pinned)))
+
+
+def dlo_set_cuts(h, cut):
+    _chk(lib().dlo_set_cuts(h, _p(cut)))
 
 
 def dlo_set_primitives(h, types_host, params):
@@ -255,6 +259,8 @@ class DloSim:
             self.h = dlo_create(self.ccfg, mat, self.stream)
             if problem.get("pins") is not None:
                 dlo_set_pins(self.h, self._up(problem["pins"][sel], torch.uint8))
+            if problem.get("cuts") is not None:
+                dlo_set_cuts(self.h, self._up(problem["cuts"][sel], torch.uint8))
             if self.K > 0:
                 dlo_set_primitives(self.h, problem["prim_types"], self._up(problem["prim_params"][sel]))
             if self.G > 0:

@@ -36,7 +36,7 @@ struct dlo_sim {
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
   float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
-  uint8_t *kin = nullptr, *pins = nullptr, *tape_flag = nullptr, *tape_flag2 = nullptr;
+  uint8_t *kin = nullptr, *pins = nullptr, *cuts = nullptr /* absent edges, allocated by dlo_set_cuts */, *tape_flag = nullptr, *tape_flag2 = nullptr;
   float* side[2] = {nullptr, nullptr};   // side-record pools, slot counters and slot indices of the two tape buffers
   int *side_count[2] = {nullptr, nullptr}, *tape_slot[2] = {nullptr, nullptr};
   int side_cap = 0, side_floats = 0;
@@ -288,7 +288,7 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   MatArgs ma;
   for (int k = 0; k < MAT_N; ++k) ma.a[k] = mp[k];
   k_pack_material<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, ma, s->mat);
-  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->kin);
+  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->cuts, s->kin);
   s->launches += 2;
   CUD(cudaGetLastError());
   CUD(cudaStreamSynchronize(s->stream));   // the material arrays are the caller's: done with them before returning
@@ -306,7 +306,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
   if (cur != s->device) cudaSetDevice(s->device);   // free on the handle's own device, whatever is current
   cudaStreamSynchronize(s->stream);
   void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->side[0], s->side[1], s->side_count[0], s->side_count[1], s->tape_slot[0], s->tape_slot[1], s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
+                 s->kin, s->pins, s->cuts, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->side[0], s->side[1], s->side_count[0], s->side_count[1], s->tape_slot[0], s->tape_slot[1], s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
   for (void* p : dev) if (p) cudaFree(p);
   if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
   for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
@@ -322,7 +322,7 @@ dlo_status dlo_destroy(dlo_sim* s) {
 
 static dlo_status rebuild_kin(dlo_sim* s) {
   const KParams& P = s->P;
-  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->kin);
+  k_build_kin<<<(P.B + 127) / 128, 128, 0, s->stream>>>(P.B, P.N, P.NS, P.G, P.M, s->pins, s->grasp, s->cuts, s->kin);
   s->launches += 1;
   CU(cudaGetLastError());
   s->have_state = false; s->have_q = false;
@@ -333,6 +333,16 @@ dlo_status dlo_set_pins(dlo_sim* s, const uint8_t* pinned) {
   ENTER(s);
   if (!pinned) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
   CU(cudaMemcpyAsync(s->pins, pinned, (size_t)s->P.B * s->P.N, cudaMemcpyDeviceToDevice, s->stream));
+  return rebuild_kin(s);
+}
+
+dlo_status dlo_set_cuts(dlo_sim* s, const uint8_t* cut) {
+  ENTER(s);
+  if (!cut) return fail(DLO_ERR_INVALID_ARG, "NULL argument");
+  if (s->P.ring) return fail(DLO_ERR_UNSUPPORTED, "dlo_set_cuts needs the open topology (the ropes lie back to back in one vertex array)");
+  if (s->P.self_contact && s->P.self_skip != 2) return fail(DLO_ERR_UNSUPPORTED, "dlo_set_cuts with self-contact needs self_skip == 2");
+  if (!s->cuts) CU(dalloc(&s->cuts, (size_t)s->P.B * s->P.N));
+  CU(cudaMemcpyAsync(s->cuts, cut, (size_t)s->P.B * s->P.N, cudaMemcpyDeviceToDevice, s->stream));
   return rebuild_kin(s);
 }
 
@@ -371,7 +381,7 @@ dlo_status dlo_set_state(dlo_sim* s, const float* x0, const float* v0, const flo
   if (P.G > 0 && !s->have_grippers) return fail(DLO_ERR_BAD_STATE, "dlo_set_grippers must precede dlo_set_state");
   SetupArgs A;
   A.B = P.B; A.N = P.N; A.E = P.E; A.NS = P.NS; A.ring = P.ring; A.G = P.G; A.M = P.M; A.kappa_from_x0 = s->cfg.kappa_bar_from_x0;
-  A.x0 = x0; A.v0 = v0; A.kb0 = kb0; A.pose0 = s->pose0; A.grasp_verts = s->grasp; A.state = s->state0; A.qloc = s->qloc;
+  A.x0 = x0; A.v0 = v0; A.kb0 = kb0; A.pose0 = s->pose0; A.grasp_verts = s->grasp; A.state = s->state0; A.qloc = s->qloc; A.cuts = s->cuts;
   k_set_state<<<(P.B + 63) / 64, 64, 0, s->stream>>>(A);
   s->launches += 1;
   CU(cudaGetLastError());

@@ -108,11 +108,11 @@ dlo_status dlo_rollout_forward_static(const dlo_config* cfg, const dlo_material*
   MatArgs ma;
   for (int k = 0; k < MAT_N; ++k) ma.a[k] = mp[k];
   k_pack_material<<<(P.B + 127) / 128, 128, 0, st>>>(P.B, ma, d_mat);
-  k_build_kin<<<(P.B + 127) / 128, 128, 0, st>>>(P.B, P.N, P.NS, P.G, P.M, scene ? scene->pinned : nullptr, P.G > 0 ? scene->grasp_verts : nullptr, d_kin);
+  k_build_kin<<<(P.B + 127) / 128, 128, 0, st>>>(P.B, P.N, P.NS, P.G, P.M, scene ? scene->pinned : nullptr, P.G > 0 ? scene->grasp_verts : nullptr, nullptr, d_kin);
   SetupArgs A;
   A.B = P.B; A.N = P.N; A.E = P.E; A.NS = P.NS; A.ring = P.ring; A.G = P.G; A.M = P.M; A.kappa_from_x0 = cfg->kappa_bar_from_x0;
   A.x0 = x0; A.v0 = v0; A.kb0 = kappa_bar0; A.pose0 = P.G > 0 ? scene->init_pose : nullptr; A.grasp_verts = P.G > 0 ? scene->grasp_verts : nullptr;
-  A.state = d_state; A.qloc = d_qloc;
+  A.state = d_state; A.qloc = d_qloc; A.cuts = nullptr;
   k_set_state<<<(P.B + 63) / 64, 64, 0, st>>>(A);
   CU(cudaGetLastError());
   P.mat = d_mat; P.kin = d_kin; P.qloc = d_qloc; P.state = d_state; P.flags = d_flags;

@@ -22,6 +22,7 @@ struct SetupArgs {
   const float *x0, *v0, *kb0;      // user arrays [B][3][N], [B][2][N] (kb0 may be null)
   const float* pose0;              // [B][G][6]
   const int* grasp_verts;          // [B][G][M]
+  const uint8_t* cuts;             // [B][N] absent edges (dlo_set_cuts) or null
   float* state;                    // [B][11][NS]
   float* qloc;                     // [B][G*M][3]
 };
@@ -44,12 +45,17 @@ __global__ void k_set_state(SetupArgs A) {
   auto xv = [&](int i) { return mk3<double>((double)X[i], (double)X[N + i], (double)X[2 * N + i]); };
   auto tang = [&](int j) { d3 e = xv((j + 1 < N) ? j + 1 : 0) - xv(j); return (1.0 / sqrt(dot(e, e))) * e; };
   auto put_d1 = [&](int j, const d3& d) { S[(ROW_D1 + 0) * NS + j] = (float)d.x; S[(ROW_D1 + 1) * NS + j] = (float)d.y; S[(ROW_D1 + 2) * NS + j] = (float)d.z; };
-  d3 t0 = tang(0);
+  const uint8_t* cut = A.cuts ? A.cuts + (size_t)env * N : nullptr;   // several DLOs: every rope starts a frame chain of its own
+  auto absent = [&](int j) { return cut && cut[j] != 0; };
   d3 zhat = mk3<double>(0, 0, 1), yhat = mk3<double>(0, 1, 0);
-  d3 cz = cross(t0, zhat);
-  d3 ref = (sqrt(dot(cz, cz)) < 1e-6) ? yhat : zhat;
-  d3 u = ref - dot(ref, t0) * t0;
-  d3 d0 = (1.0 / sqrt(dot(u, u))) * u, d = d0, tp = t0;
+  auto first_director = [&](const d3& t) {
+    d3 cz = cross(t, zhat);
+    d3 ref = (sqrt(dot(cz, cz)) < 1e-6) ? yhat : zhat;
+    d3 u = ref - dot(ref, t) * t;
+    return (1.0 / sqrt(dot(u, u))) * u;
+  };
+  d3 t0 = tang(0);
+  d3 d0 = first_director(t0), d = d0, tp = t0;
   double psiH = 0.0;
   if (A.ring) {   // first pass: holonomy of the closed loop
     for (int j = 1; j < E; ++j) { d3 tj = tang(j); d = ptransport<double>(tp, tj, d); tp = tj; }
@@ -57,9 +63,12 @@ __global__ void k_set_state(SetupArgs A) {
     psiH = atan2(dot(cross(d0, uu), t0), dot(d0, uu));
     d = d0; tp = t0;
   }
+  bool fresh = false;
   for (int j = 0; j < E; ++j) {
+    if (absent(j)) { fresh = true; continue; }   // no frame on an absent edge (the row stays zero)
     d3 tj = tang(j);
-    if (j > 0) { d = ptransport<double>(tp, tj, d); tp = tj; }
+    if (fresh) { d = first_director(tj); tp = tj; fresh = false; }
+    else if (j > 0) { d = ptransport<double>(tp, tj, d); tp = tj; }
     d3 out = d;
     if (A.ring) {   // Eq.12: rotate by phi^j = -psiH * j / E about the tangent
       const double phi = -psiH * (double)j / (double)E;
@@ -73,6 +82,7 @@ __global__ void k_set_state(SetupArgs A) {
   } else if (A.kappa_from_x0) {
     for (int i = 0; i < N; ++i) {
       if (!(A.ring || (i >= 1 && i <= N - 2))) continue;
+      if (absent(i - 1 >= 0 ? i - 1 : 0) || absent(i)) continue;   // a rope end has no bending element
       const int a = (i + N - 1) % N;
       d3 da = mk3<double>(S[ROW_D1 * NS + a], S[(ROW_D1 + 1) * NS + a], S[(ROW_D1 + 2) * NS + a]);
       d3 db = mk3<double>(S[ROW_D1 * NS + i], S[(ROW_D1 + 1) * NS + i], S[(ROW_D1 + 2) * NS + i]);
@@ -95,7 +105,7 @@ __global__ void k_set_state(SetupArgs A) {
 }
 
 // kinematic codes from pins and grasp sets (grasp flags on top of pins, like the problem statement R-19)
-__global__ void k_build_kin(int B, int N, int NS, int G, int M, const uint8_t* pins, const int* grasp_verts, uint8_t* kin) {
+__global__ void k_build_kin(int B, int N, int NS, int G, int M, const uint8_t* pins, const int* grasp_verts, const uint8_t* cuts, uint8_t* kin) {
   const int env = blockIdx.x * blockDim.x + threadIdx.x;
   if (env >= B) return;
   uint8_t* K = kin + (size_t)env * NS;
@@ -106,6 +116,9 @@ __global__ void k_build_kin(int B, int N, int NS, int G, int M, const uint8_t* p
         const int v = grasp_verts[((size_t)env * G + g) * M + k];
         if (v >= 0 && v < N) K[v] = (uint8_t)(KIN_GRASP0 + g * M + k);
       }
+  if (cuts)
+    for (int i = 0; i < N; ++i)
+      if (cuts[(size_t)env * N + i]) K[i] |= KIN_CUT;
 }
 
 struct MatArgs { const float* a[MAT_N]; };

@@ -229,7 +229,7 @@ __device__ __noinline__ int build_pair_list(const KParams& __restrict__ P, int l
   unsigned mymask = 0u;
   for (int A = 0; A < nb; ++A) {
     const float dx = sm.blk[A] - bx, dy = sm.blk[32 + A] - by, dz = sm.blk[64 + A] - bz, reach = sm.blk[96 + A] + br + lim;
-    const bool hit = lane >= A && lane < nb && dx * dx + dy * dy + dz * dz < reach * reach;
+    const bool hit = lane >= A && lane < nb && reach > 0.0f && dx * dx + dy * dy + dz * dz < reach * reach;   // (a block of absent edges has radius -1e30)
     const unsigned m = __ballot_sync(DLO_FULL, hit);
     if (lane == A) mymask = m;
   }
@@ -250,7 +250,7 @@ __device__ __noinline__ int build_pair_list(const KParams& __restrict__ P, int l
           const int pa = vpos<VPL>(a), pb = vpos<VPL>(b);
           const float dx = sm.mid[pb] - sm.mid[pa], dy = sm.mid[NP + pb] - sm.mid[NP + pa], dz = sm.mid[2 * NP + pb] - sm.mid[2 * NP + pa];
           const float reach = sm.mid[3 * NP + pa] + sm.mid[3 * NP + pb] + lim;
-          hit = dx * dx + dy * dy + dz * dz < reach * reach;
+          hit = reach > 0.0f && dx * dx + dy * dy + dz * dz < reach * reach;
         }
         const unsigned m = __ballot_sync(DLO_FULL, hit);
         if (hit) {
@@ -631,7 +631,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
         const int i = vpos<VPL>(tp.base + k);
         sts3(sm.xref, sm.NP, i, XP(k));
         sts3(sm.mid, sm.NP, i, axpy(XP(k), 0.5f, epred[k]));
-        sm.mid[3 * sm.NP + i] = 0.5f * sqrt_(dot(epred[k], epred[k]));
+        sm.mid[3 * sm.NP + i] = tp.evalid[k] ? 0.5f * sqrt_(dot(epred[k], epred[k])) : -1.0e30f;   // an absent edge (cut) is in reach of nothing
       }
       // bounding sphere of this lane's edge block (centre = mean of its edge midpoints)
       f3 bc = zero3<float>();

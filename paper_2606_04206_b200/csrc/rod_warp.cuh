@@ -16,6 +16,7 @@ namespace dlo {
 
 typedef V3<float> f3;
 enum { KIN_FREE = 0, KIN_PINNED = 1, KIN_GRASP0 = 2 };   // kin code >= 2: grasped, slot = code - 2 = g*M + k
+enum { KIN_CUT = 0x80 };   // bit 7 of the kin byte of vertex i: the edge (i, i+1) does not exist (several DLOs in one env, dlo_set_cuts)
 enum { MAT_M = 0, MAT_L0, MAT_STRETCH, MAT_ALPHA, MAT_GAMMA, MAT_SIGY, MAT_RC, MAT_MUR, MAT_MUS, MAT_N };
 // rows of one env's state block.  Positions are kept as an unevaluated sum x + xl of two floats (xl = what the fp32 rounding
 // of x + h v dropped, |xl| <= ulp(x)/2): an fp32 position at 0.5 m carries 3e-8 m of rounding, which the next substep's Eq.10
@@ -217,14 +218,27 @@ template <int VPL> struct EnvConst {
   float wr;           // inverse mass of the remote next vertex (slot 0 of lane nl)
 };
 
-template <int VPL> __device__ __forceinline__ void load_env(const KParams& P, int env, const Topo<VPL>& tp, EnvConst<VPL>& c) {
+template <int VPL> __device__ __forceinline__ void load_env(const KParams& P, int env, Topo<VPL>& tp, EnvConst<VPL>& c) {
   const float* M = P.mat + (size_t)env * MAT_N;
   c.m = M[MAT_M]; c.inv_m = 1.0f / c.m; c.l0 = M[MAT_L0]; c.stretch = M[MAT_STRETCH]; c.alpha = M[MAT_ALPHA];
   c.gamma = M[MAT_GAMMA]; c.sigy = M[MAT_SIGY]; c.rc = M[MAT_RC]; c.mu_r = M[MAT_MUR]; c.mu_s = M[MAT_MUS];
+  bool cut[VPL];
 #pragma unroll
   for (int k = 0; k < VPL; ++k) {
-    c.kin[k] = tp.vvalid[k] ? (int)P.kin[(size_t)env * P.NS + tp.base + k] : KIN_PINNED;
+    const int raw = tp.vvalid[k] ? (int)P.kin[(size_t)env * P.NS + tp.base + k] : KIN_PINNED;
+    c.kin[k] = raw & (KIN_CUT - 1);
+    cut[k] = (raw & KIN_CUT) != 0;
     c.w[k] = (tp.vvalid[k] && c.kin[k] == KIN_FREE) ? c.inv_m : 0.0f;
+  }
+  // several DLOs in one env: an absent edge is no edge (no stretch / Eq.10 constraint, no frame, no contact segment), and a
+  // vertex next to it is a rope end (no bending element).  The previous lane is always full: its last slot is VPL - 1.
+  {
+    const bool prev_cut = __shfl_sync(DLO_FULL, (int)cut[VPL - 1], tp.pl) != 0;
+#pragma unroll
+    for (int k = 0; k < VPL; ++k) {
+      if (cut[k]) tp.evalid[k] = false;
+      if (cut[k] || (k == 0 ? prev_cut : cut[k > 0 ? k - 1 : 0])) tp.interior[k] = false;
+    }
   }
   c.wr = shfl(c.w[0], tp.nl);
   // opaque from here on: otherwise the compiler, short of registers, re-derives w[k] from kin[k], the lane index and N at

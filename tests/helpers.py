@@ -4,8 +4,9 @@ import numpy as np
 from workloads.configs import DEFAULTS, _material
 
 
-def rope_problem(x0, v0=None, *, ring=False, dt=1e-3, horizon=10, stride=0, material=None, pins=None, **cfg_over):
-    """Problem dict for a batch of ropes given as x0 [B][N][3] (AoS for convenience)."""
+def rope_problem(x0, v0=None, *, ring=False, dt=1e-3, horizon=10, stride=0, material=None, pins=None, cuts=None, **cfg_over):
+    """Problem dict for a batch of ropes given as x0 [B][N][3] (AoS for convenience).  cuts: vertex indices j whose edge
+    (j, j+1) does not exist (several ropes back to back in one env)."""
     x0 = np.asarray(x0, dtype=np.float64)
     if x0.ndim == 2:
         x0 = x0[None]
@@ -14,7 +15,10 @@ def rope_problem(x0, v0=None, *, ring=False, dt=1e-3, horizon=10, stride=0, mate
     cfg.update(batch=B, n_verts=N, dt=dt, topology=1 if ring else 0)
     cfg.update(cfg_over)
     E = N if ring else N - 1
-    mat = dict(l0=np.linalg.norm(np.roll(x0, -1, axis=1) - x0, axis=2)[:, :E].mean(axis=1))
+    keep = np.ones(E, dtype=bool)
+    if cuts is not None:
+        keep[list(cuts)] = False
+    mat = dict(l0=np.linalg.norm(np.roll(x0, -1, axis=1) - x0, axis=2)[:, :E][:, keep].mean(axis=1))
     mat.update(material or {})
     P = dict(config=cfg, horizon=horizon, checkpoint_stride=stride, pins=None, kappa_bar0=None, actions=None)
     P["material"] = _material(B, **mat)
@@ -24,6 +28,10 @@ def rope_problem(x0, v0=None, *, ring=False, dt=1e-3, horizon=10, stride=0, mate
         p = np.zeros((B, N), dtype=np.uint8)
         p[:, list(pins)] = 1
         P["pins"] = p
+    if cuts is not None:
+        c = np.zeros((B, N), dtype=np.uint8)
+        c[:, list(cuts)] = 1
+        P["cuts"] = c
     return P
 
 

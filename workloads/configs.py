@@ -357,7 +357,7 @@ def subset(problem, envs):
     Q = dict(problem)
     Q["config"] = dict(problem["config"], batch=len(envs))
     Q["material"] = {k: v[envs] for k, v in problem["material"].items()}
-    for k in ("pins", "prim_params", "init_pose", "finger_geom", "grasp_verts", "x0", "v0", "kappa_bar0"):
+    for k in ("pins", "cuts", "prim_params", "init_pose", "finger_geom", "grasp_verts", "x0", "v0", "kappa_bar0"):
         if problem.get(k) is not None:
             Q[k] = problem[k][envs]
     if problem.get("actions") is not None:
