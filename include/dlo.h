@@ -160,7 +160,10 @@ dlo_status dlo_backward_host(dlo_sim* sim, const float* dL_dx_T, const float* dL
  * candidate list since dlo_set_state; n_bad (host, may be NULL) receives the number of such envs. */
 dlo_status dlo_check_numerics(dlo_sim* sim, int32_t* n_bad);
 
-/* Device bytes the library allocates for this config / rollout shape (constants + checkpoints + tape).  A handle that
+/* Device bytes the library allocates for this config / rollout shape (constants + checkpoints + tape; the tape of one
+ * checkpoint segment, twice when there are several).  While more than a tenth of the device's memory stays free the handle
+ * takes up to two more tape buffers of the same size (DLO_TAPE_BUFFERS = 1..4 caps the total): the forward rollout then
+ * leaves its last segments on tape and the reverse pass skips their replay.  A handle that
  * is driven through the *_host calls additionally holds their device staging: 4 + 4 arrays [B][3][N], one [B][2][N],
  * one [B][5] and two [H][B][G][6] (actions, action gradients). */
 size_t dlo_scratch_bytes(const dlo_config* cfg, int32_t horizon, int32_t checkpoint_stride);

@@ -36,23 +36,30 @@ struct dlo_sim {
   // library-owned device memory
   float *mat = nullptr, *qloc = nullptr, *pose0 = nullptr, *finger = nullptr, *prim = nullptr;
   float *state = nullptr, *state0 = nullptr, *ckpt = nullptr, *tape = nullptr, *acc_tape = nullptr, *adj = nullptr, *replay = nullptr, *gmat = nullptr;
-  uint8_t *kin = nullptr, *pins = nullptr, *cuts = nullptr /* absent edges, allocated by dlo_set_cuts */, *tape_flag = nullptr, *tape_flag2 = nullptr;
-  float* side[2] = {nullptr, nullptr};   // side-record pools, slot counters and slot indices of the two tape buffers
-  int *side_count[2] = {nullptr, nullptr}, *tape_slot[2] = {nullptr, nullptr};
+  uint8_t *kin = nullptr, *pins = nullptr, *cuts = nullptr /* absent edges, allocated by dlo_set_cuts */;
+  // Tape buffers, one checkpoint segment each (n_tape of them, segment g uses buffer g % n_tape).  The first is required; the
+  // others are taken while device memory allows (180 GB of HBM: config 5 fits four of its ten 37 GB segments).  The forward
+  // rollout writes the tape of its LAST n_tape segments itself, so the reverse pass replays only the segments before them,
+  // and with more than one buffer those replays run on a second stream under the adjoint of a later segment.
+  enum { MAX_TAPE = 4 };
+  float* tapes[MAX_TAPE] = {};
+  uint8_t* tape_flags[MAX_TAPE] = {};
+  float* side[MAX_TAPE] = {};          // side-record pools, slot counters and slot indices, per tape buffer
+  int *side_count[MAX_TAPE] = {}, *tape_slot[MAX_TAPE] = {};
   int side_cap = 0, side_floats = 0;
-  float* tape2 = nullptr;            // second tape buffer: the replay of segment g-1 overlaps the adjoint of segment g
+  int n_tape = 0, max_tape = MAX_TAPE;   // allocated / wanted at most (DLO_TAPE_BUFFERS)
   cudaStream_t aux = nullptr;
-  cudaEvent_t ev_fwd = nullptr, ev_rep[2] = {nullptr, nullptr}, ev_adj[2] = {nullptr, nullptr};
+  cudaEvent_t ev_fwd = nullptr, ev_rep[MAX_TAPE] = {}, ev_adj[MAX_TAPE] = {};
   int *grasp = nullptr, *flags = nullptr;
   // env -> warp-slot order (k_sort_envs): work statistics of the last forward chunk / of the tape in each tape buffer, the orders made from them
-  int *stat = nullptr, *stat_rep[2] = {nullptr, nullptr}, *perm_main = nullptr, *perm_rep = nullptr;
-  bool stat_valid = false, stat_rep_valid[2] = {false, false};
+  int *stat = nullptr, *stat_rep[MAX_TAPE] = {}, *perm_main = nullptr, *perm_rep = nullptr;
+  bool stat_valid = false, stat_rep_valid[MAX_TAPE] = {};
   int chunk = 100;                 // frames per forward launch when the forward re-orders (sort_mode bit 0)
   int sort_mode = 6;               // bit 0: forward launches, bit 1: replays, bit 2: adjoint launches take the envs in sorted order
   size_t ckpt_blocks = 0, tape_blocks = 0;
   const float* actions = nullptr;   // borrowed
   int H_actions = 0, H_done = 0, stride = 0;
-  int tape_seg = -1, tape_buf = 0;  // segment whose tape records are in a buffer already (written by the forward rollout), and which buffer
+  int tape_lo = 1 << 30, tape_K = 0;   // segments >= tape_lo of the last forward rollout are on tape already, segment g in buffer g % tape_K
   int device = 0;                  // the CUDA device the handle was created on (every call must be made with it current)
   int t_start = 0;                 // frame index of state0 (0 after dlo_set_state; dlo_restore_state sets it)
   bool have_state = false, have_q = false, have_prims = false, have_grippers = false, have_adj = false;
@@ -274,7 +281,9 @@ dlo_status dlo_create(const dlo_config* cfg, const dlo_material* mat, void* stre
   CUD(dalloc(&s->state, B * s->blk));
   CUD(dalloc(&s->state0, B * s->blk));
   CUD(dalloc(&s->flags, B));
-  CUD(dalloc(&s->stat, 2 * B)); CUD(dalloc(&s->stat_rep[0], 2 * B)); CUD(dalloc(&s->stat_rep[1], 2 * B));
+  CUD(dalloc(&s->stat, 2 * B));
+  for (int k = 0; k < dlo_sim::MAX_TAPE; ++k) CUD(dalloc(&s->stat_rep[k], 2 * B));
+  if (const char* ov = getenv("DLO_TAPE_BUFFERS")) s->max_tape = std::max(1, std::min((int)dlo_sim::MAX_TAPE, atoi(ov)));   // tuning override (no effect on results)
   CUD(dalloc(&s->perm_main, B)); CUD(dalloc(&s->perm_rep, B));
   if (const char* ov = getenv("DLO_CHUNK")) s->chunk = std::max(1, atoi(ov));   // tuning overrides (no effect on results)
   if (const char* ov = getenv("DLO_SORT")) s->sort_mode = atoi(ov) & 7;
@@ -305,11 +314,16 @@ dlo_status dlo_destroy(dlo_sim* s) {
   cudaGetDevice(&cur);
   if (cur != s->device) cudaSetDevice(s->device);   // free on the handle's own device, whatever is current
   cudaStreamSynchronize(s->stream);
-  void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->tape, s->acc_tape, s->adj, s->replay, s->gmat,
-                 s->kin, s->pins, s->cuts, s->grasp, s->flags, s->tape_flag, s->tape_flag2, s->tape2, s->side[0], s->side[1], s->side_count[0], s->side_count[1], s->tape_slot[0], s->tape_slot[1], s->stat, s->stat_rep[0], s->stat_rep[1], s->perm_main, s->perm_rep};
+  if (s->aux) cudaStreamSynchronize(s->aux);
+  void* dev[] = {s->mat, s->qloc, s->pose0, s->finger, s->prim, s->state, s->state0, s->ckpt, s->acc_tape, s->adj, s->replay, s->gmat,
+                 s->kin, s->pins, s->cuts, s->grasp, s->flags, s->stat, s->perm_main, s->perm_rep};
   for (void* p : dev) if (p) cudaFree(p);
-  if (s->aux) { cudaStreamSynchronize(s->aux); cudaStreamDestroy(s->aux); }
-  for (cudaEvent_t e : {s->ev_fwd, s->ev_rep[0], s->ev_rep[1], s->ev_adj[0], s->ev_adj[1]}) if (e) cudaEventDestroy(e);
+  for (int k = 0; k < dlo_sim::MAX_TAPE; ++k) {
+    for (void* p : {(void*)s->tapes[k], (void*)s->tape_flags[k], (void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k], (void*)s->stat_rep[k]}) if (p) cudaFree(p);
+    for (cudaEvent_t e : {s->ev_rep[k], s->ev_adj[k]}) if (e) cudaEventDestroy(e);
+  }
+  if (s->aux) cudaStreamDestroy(s->aux);
+  if (s->ev_fwd) cudaEventDestroy(s->ev_fwd);
   for (auto& v : s->tev) for (cudaEvent_t e : v) cudaEventDestroy(e);
   void* stg[] = {s->dx0, s->dv0, s->dkb, s->dact, s->dxT, s->dvT, s->dsx, s->dsv, s->dga, s->dgx, s->dgv, s->dgm};
   for (void* p : stg) if (p) cudaFree(p);
@@ -474,48 +488,63 @@ static cudaError_t forward_chunks(dlo_sim* s, int t0, int t1, int stride) {
   return cudaSuccess;
 }
 
-// tape buffers of one checkpoint segment (two when there are several segments and memory allows: DESIGN.md section 5)
+// Tape buffers, one checkpoint segment each: the first is required, up to min(#segments, max_tape) are taken while memory
+// allows.  Each comes with its optional side-record pool.
+static void free_tape_buffer(dlo_sim* s, int k) {
+  for (void* p : {(void*)s->tapes[k], (void*)s->tape_flags[k], (void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
+  s->tapes[k] = nullptr; s->tape_flags[k] = nullptr; s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
+}
 static dlo_status ensure_tape(dlo_sim* s, int H, int stride) {
   const int B = s->P.B;
   const size_t rec = (size_t)tape_rows(s->P.N_C) * s->P.NS, seg = (size_t)(stride < H ? stride : H) * s->P.n_sub + 1;
   const int nseg = (H + stride - 1) / stride;
-  if (seg > s->tape_blocks) {
+  if (seg > s->tape_blocks) {   // a longer segment than the buffers hold: start over
     CU(cudaStreamSynchronize(s->stream));
     if (s->aux) CU(cudaStreamSynchronize(s->aux));
-    for (void* p : {(void*)s->tape, (void*)s->tape2, (void*)s->tape_flag, (void*)s->tape_flag2}) if (p) cudaFree(p);
-    s->tape = s->tape2 = nullptr; s->tape_flag = s->tape_flag2 = nullptr; s->tape_blocks = 0;
-    CU(dalloc(&s->tape, seg * B * rec));
-    CU(dalloc(&s->tape_flag, seg * B));
+    for (int k = 0; k < dlo_sim::MAX_TAPE; ++k) free_tape_buffer(s, k);
+    s->n_tape = 0; s->tape_blocks = 0; s->side_cap = 0;
+    s->tape_lo = 1 << 30;
+    CU(dalloc(&s->tapes[0], seg * B * rec));
+    CU(dalloc(&s->tape_flags[0], seg * B));
     s->tape_blocks = seg;
-    for (int k = 0; k < 2; ++k) {
-      for (void* p : {(void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
-      s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
-    }
-    s->side_cap = 0;
+    s->n_tape = 1;
   }
-  if (s->P.self_contact && !getenv("DLO_NO_SIDE")) {
+  const bool want_side = s->P.self_contact && !getenv("DLO_NO_SIDE");
+  if (want_side) {
     // side records for one substep in twelve (config 5 uses one in thirty); a substep that finds the pool empty is
     // recomputed by the reverse pass instead.  Optional: without the memory the reverse pass recomputes them all.
     s->side_floats = side_record_floats(s->P, 33 * s->VPL);
     s->side_cap = (int)std::min<size_t>((size_t)1 << 30, std::max<size_t>(1024, s->tape_blocks * B / 12));
-    for (int k = 0; k < (nseg > 1 ? 2 : 1); ++k) {
-      if (s->side[k]) continue;
-      const bool ok = cudaMalloc((void**)&s->side[k], (size_t)s->side_cap * s->side_floats * sizeof(float)) == cudaSuccess &&
-                      cudaMalloc((void**)&s->side_count[k], sizeof(int)) == cudaSuccess &&
-                      cudaMalloc((void**)&s->tape_slot[k], s->tape_blocks * B * sizeof(int)) == cudaSuccess;
-      if (!ok) {
-        cudaGetLastError();
-        for (void* p : {(void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
-        s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
-      }
-    }
   }
-  if (nseg > 1 && !s->tape2) {
-    if (cudaMalloc((void**)&s->tape2, s->tape_blocks * B * rec * sizeof(float)) != cudaSuccess ||
-        cudaMalloc((void**)&s->tape_flag2, s->tape_blocks * B) != cudaSuccess) {
+  auto side_pool = [&](int k) {
+    if (!want_side || s->side[k]) return;
+    const bool ok = cudaMalloc((void**)&s->side[k], (size_t)s->side_cap * s->side_floats * sizeof(float)) == cudaSuccess &&
+                    cudaMalloc((void**)&s->side_count[k], sizeof(int)) == cudaSuccess &&
+                    cudaMalloc((void**)&s->tape_slot[k], s->tape_blocks * B * sizeof(int)) == cudaSuccess;
+    if (!ok) {
       cudaGetLastError();
-      if (s->tape2) { cudaFree(s->tape2); s->tape2 = nullptr; }
+      for (void* p : {(void*)s->side[k], (void*)s->side_count[k], (void*)s->tape_slot[k]}) if (p) cudaFree(p);
+      s->side[k] = nullptr; s->side_count[k] = nullptr; s->tape_slot[k] = nullptr;
     }
+  };
+  side_pool(0);
+  const int want = std::min(nseg, s->max_tape);
+  const size_t tape_bytes = s->tape_blocks * B * rec * sizeof(float);
+  const size_t side_bytes = want_side ? (size_t)s->side_cap * s->side_floats * sizeof(float) + s->tape_blocks * B * sizeof(int) : 0;
+  while (s->n_tape < want) {
+    const int k = s->n_tape;
+    if (k >= 2) {   // beyond double buffering: only out of memory nobody else is likely to need (a tenth of the device stays free)
+      size_t free_b = 0, total_b = 0;
+      if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); break; }
+      if (free_b < tape_bytes + side_bytes + total_b / 10) break;
+    }
+    if (cudaMalloc((void**)&s->tapes[k], tape_bytes) != cudaSuccess || cudaMalloc((void**)&s->tape_flags[k], s->tape_blocks * B) != cudaSuccess) {
+      cudaGetLastError();
+      free_tape_buffer(s, k);
+      break;
+    }
+    side_pool(k);
+    s->n_tape = k + 1;
   }
   return DLO_OK;
 }
@@ -545,30 +574,32 @@ dlo_status dlo_rollout_forward(dlo_sim* s, int32_t horizon, int32_t stride) {
     s->P.ckpt = s->ckpt;
     CU(cudaMemcpyAsync(s->ckpt, s->state0, blk_bytes, cudaMemcpyDeviceToDevice, s->stream));   // checkpoint 0 = initial state
   }
-  s->tape_seg = -1;
-  s->stat_valid = s->stat_rep_valid[0] = s->stat_rep_valid[1] = false;
+  s->tape_lo = 1 << 30; s->tape_K = 0;
+  s->stat_valid = false;
+  for (bool& v : s->stat_rep_valid) v = false;
   if (horizon > 0 && stride > 0) {
-    // the last segment is run in tape mode, so that the reverse pass can start without replaying it
+    // the last n_tape segments are run in tape mode, so that the reverse pass can start without replaying them
     dlo_status st = ensure_tape(s, horizon, stride);
     if (st) return st;
-    const int nseg = (horizon + stride - 1) / stride, t_last = (nseg - 1) * stride;
-    const bool two = nseg > 1 && s->tape2 && s->tape_flag2;
-    if (t_last > 0) CU(forward_chunks(s, 0, t_last, stride));
-    KParams Pf = s->P;
-    const int buf = (two && ((nseg - 1) & 1)) ? 1 : 0;
-    Pf.tape = buf ? s->tape2 : s->tape;
-    Pf.tape_flag = buf ? s->tape_flag2 : s->tape_flag;
-    if (s->side[buf]) {
-      CU(cudaMemsetAsync(s->side_count[buf], 0, sizeof(int), s->stream));
-      Pf.side = s->side[buf]; Pf.side_count = s->side_count[buf]; Pf.tape_slot = s->tape_slot[buf]; Pf.side_cap = s->side_cap; Pf.side_floats = s->side_floats;
+    const int nseg = (horizon + stride - 1) / stride, K = s->n_tape, lo = nseg - std::min(K, nseg);
+    if (lo > 0) CU(forward_chunks(s, 0, lo * stride, stride));
+    for (int g = lo; g < nseg; ++g) {
+      const int buf = g % K, t0 = g * stride, t1 = std::min(t0 + stride, (int)horizon);
+      KParams Pf = s->P;
+      Pf.tape = s->tapes[buf];
+      Pf.tape_flag = s->tape_flags[buf];
+      if (s->side[buf]) {
+        CU(cudaMemsetAsync(s->side_count[buf], 0, sizeof(int), s->stream));
+        Pf.side = s->side[buf]; Pf.side_count = s->side_count[buf]; Pf.tape_slot = s->tape_slot[buf]; Pf.side_cap = s->side_cap; Pf.side_floats = s->side_floats;
+      }
+      if (s->sort_mode) {
+        Pf.stat = s->stat_rep[buf];
+        if ((s->sort_mode & 1) && s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }
+      }
+      CU(launch_forward(s, Pf, t0, t1, stride, true, s->stream));
+      s->stat_rep_valid[buf] = s->sort_mode != 0;
     }
-    if (s->sort_mode) {
-      Pf.stat = s->stat_rep[buf];
-      if ((s->sort_mode & 1) && s->stat_valid) { CU(sort_envs(s, s->stat, 0, 4, s->perm_main, s->stream)); Pf.perm = s->perm_main; }
-    }
-    CU(launch_forward(s, Pf, t_last, horizon, stride, true, s->stream));
-    s->stat_rep_valid[buf] = s->sort_mode != 0;
-    s->tape_seg = nseg - 1; s->tape_buf = buf;
+    s->tape_lo = lo; s->tape_K = K;
   } else if (horizon > 0) CU(forward_chunks(s, 0, horizon, stride));
   s->H_done = horizon; s->stride = stride;
   return DLO_OK;

@@ -48,34 +48,46 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
   CU(cudaMemsetAsync(s->gmat, 0, (size_t)B * 5 * sizeof(float), s->stream));
   if (g_actions && s->P.G > 0) CU(cudaMemsetAsync(g_actions, 0, (size_t)H * B * s->P.G * 6 * sizeof(float), s->stream));
   const int nseg = (H + stride - 1) / stride;
-  // Two tape buffers when there is more than one segment and memory allows: the replay of segment g-1 (auxiliary stream)
-  // then overlaps the adjoint of segment g and fills the SMs its last, partly empty wave leaves idle.
-  const bool overlap = nseg > 1 && s->tape2 && s->tape_flag2;
+  // K tape buffers, segment g in buffer g % K.  The forward rollout left its last K segments on tape; every other segment
+  // is replayed from its checkpoint first.  With K > 1 the replays run on a second stream: the replay of segment r goes
+  // into the buffer the adjoint of segment r + K has just finished with, K - 1 adjoints before its records are needed.
+  const int K = s->n_tape;
+  const bool overlap = nseg > 1 && K > 1;
   if (overlap && !s->aux) {
     CU(cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking));
     CU(cudaEventCreateWithFlags(&s->ev_fwd, cudaEventDisableTiming));
-    for (int k = 0; k < 2; ++k) { CU(cudaEventCreateWithFlags(&s->ev_rep[k], cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&s->ev_adj[k], cudaEventDisableTiming)); }
   }
-  float* tapes[2] = {s->tape, overlap ? s->tape2 : s->tape};
-  uint8_t* tflags[2] = {s->tape_flag, overlap ? s->tape_flag2 : s->tape_flag};
+  if (overlap)
+    for (int k = 0; k < K; ++k) {
+      if (!s->ev_rep[k]) CU(cudaEventCreateWithFlags(&s->ev_rep[k], cudaEventDisableTiming));
+      if (!s->ev_adj[k]) CU(cudaEventCreateWithFlags(&s->ev_adj[k], cudaEventDisableTiming));
+    }
   cudaStream_t rs = overlap ? s->aux : s->stream;        // stream of the replays
+  // the forward rollout chose the buffers of its taped segments with the buffers it had THEN; if the set has changed since
+  // (a buffer that could not be allocated before), its records are not where this pass looks
+  const int tape_lo = (s->tape_K == K) ? s->tape_lo : nseg;
+  s->tape_lo = 1 << 30;   // the buffers are overwritten below
+  std::vector<char> issued(nseg, 0);
   auto replay = [&](int g) -> dlo_status {
-    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = overlap ? (g & 1) : 0;
+    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = g % K;
+    // the buffer's last user is segment g + K, whose adjoint has been launched on the main stream by now
+    if (overlap && g + K <= nseg - 1) CU(cudaStreamWaitEvent(s->aux, s->ev_adj[buf], 0));
     CU(cudaMemcpyAsync(s->replay, s->ckpt + (size_t)g * B * blk, nadj * sizeof(float), cudaMemcpyDeviceToDevice, rs));
     KParams Pf = s->P;
-    Pf.state = s->replay; Pf.tape = tapes[buf]; Pf.tape_flag = tflags[buf];
+    Pf.state = s->replay; Pf.tape = s->tapes[buf]; Pf.tape_flag = s->tape_flags[buf];
     if (s->side[buf]) {
       CU(cudaMemsetAsync(s->side_count[buf], 0, sizeof(int), rs));
       Pf.side = s->side[buf]; Pf.side_count = s->side_count[buf]; Pf.tape_slot = s->tape_slot[buf]; Pf.side_cap = s->side_cap; Pf.side_floats = s->side_floats;
     }
-    if (s->sort_mode) {   // envs in the order of the work the segment after this one took (the tape written last, on this stream or before ev_fwd)
-      const int src = overlap ? ((g + 1) & 1) : 0;
+    if (s->sort_mode) {   // envs in the order of the work the segment after this one took (its tape was written earlier on this stream, or before ev_fwd)
+      const int src = (g + 1) % K;
       if ((s->sort_mode & 2) && g + 1 < nseg && s->stat_rep_valid[src]) { CU(sort_envs(s, s->stat_rep[src], 0, 4, s->perm_rep, rs)); Pf.perm = s->perm_rep; }
       Pf.stat = s->stat_rep[buf];
     }
     CU(launch_forward(s, Pf, t0, t1, 0, true, rs));
     s->stat_rep_valid[buf] = s->sort_mode != 0;
     if (overlap) CU(cudaEventRecord(s->ev_rep[buf], rs));
+    issued[g] = 1;
     return DLO_OK;
   };
   if (overlap) {   // the replays read the checkpoints the forward rollout wrote on the main stream
@@ -83,24 +95,15 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     CU(cudaStreamWaitEvent(s->aux, s->ev_fwd, 0));
   }
   dlo_status rst = DLO_OK;
-  // the forward rollout chose the buffer of the last segment with the buffers it had THEN; if the set has changed since
-  // (a second tape buffer that could not be allocated before, or was lost), its records are not where this pass looks
-  if (s->tape_seg == nseg - 1 && s->tape_buf != (overlap ? ((nseg - 1) & 1) : 0)) s->tape_seg = -1;
-  if (s->tape_seg != nseg - 1 && (rst = replay(nseg - 1))) return rst;     // normally the forward rollout left it on the tape
-  const bool have_last = s->tape_seg == nseg - 1;
-  s->tape_seg = -1;
   for (int g = nseg - 1; g >= 0; --g) {
-    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = overlap ? (g & 1) : 0;
-    if (overlap) {
-      if (!(have_last && g == nseg - 1)) CU(cudaStreamWaitEvent(s->stream, s->ev_rep[buf], 0));
-      if (g > 0) {   // next replay goes into the other buffer, free once the adjoint of segment g+1 is done with it
-        if (g + 1 <= nseg - 1) CU(cudaStreamWaitEvent(s->aux, s->ev_adj[(g - 1) & 1], 0));
-        if ((rst = replay(g - 1))) return rst;
-      }
-    }
+    const int t0 = g * stride, t1 = (t0 + stride < H) ? t0 + stride : H, buf = g % K;
+    // replays that can be on their way now: this segment's own (if the forward did not tape it) and those of the K - 1 before it
+    for (int r = g; r >= 0 && r > g - K; --r)
+      if (r < tape_lo && !issued[r] && (r == g || overlap) && (rst = replay(r))) return rst;
+    if (overlap && issued[g]) CU(cudaStreamWaitEvent(s->stream, s->ev_rep[buf], 0));
     KParams Pa = s->P;
     smem_layout(Pa, s->VPL, true);
-    Pa.tape = tapes[buf]; Pa.tape_flag = tflags[buf]; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
+    Pa.tape = s->tapes[buf]; Pa.tape_flag = s->tape_flags[buf]; Pa.adj = s->adj; Pa.acc_tape = s->acc_tape; Pa.gmat = s->gmat; Pa.g_actions = (s->P.G > 0) ? g_actions : nullptr;
     if (s->side[buf]) { Pa.side = s->side[buf]; Pa.tape_slot = s->tape_slot[buf]; Pa.side_floats = s->side_floats; Pa.side_cap = s->side_cap; }
     if ((s->sort_mode & 4) && s->stat_rep_valid[buf]) {   // envs whose substeps must be recomputed (self-contact corrections) share CTAs
       CU(sort_envs(s, s->stat_rep[buf], 1, 0, s->perm_main, s->stream));
@@ -108,7 +111,6 @@ dlo_status dlo_backward(dlo_sim* s, const float* gxT, const float* gvT, float* g
     }
     CU(launch_adjoint(s, Pa, t0, t1));
     if (overlap) CU(cudaEventRecord(s->ev_adj[buf], s->stream));
-    else if (g > 0 && (rst = replay(g - 1))) return rst;
   }
   if (g_x0 || g_v0) {
     const size_t n = (size_t)B * STATE_ROWS * s->P.N;

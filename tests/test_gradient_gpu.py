@@ -122,6 +122,30 @@ def test_gradient_independent_of_stride(dlo):
             assert np.abs(o[k] - outs[0][k]).max() <= 5e-5 * np.abs(outs[0][k]).max(), k
 
 
+@pytest.mark.parametrize("cfg, H, stride", [(3, 45, 6), (5, 60, 7)])
+def test_gradient_independent_of_tape_buffers(dlo, monkeypatch, cfg, H, stride):
+    """How many checkpoint segments are kept on tape (DLO_TAPE_BUFFERS: 1 = every segment replayed on the main stream, 2 =
+    the forward tapes its last two and the other replays run under the adjoints on a second stream, 4 = the default cap)
+    is a memory / recompute trade-off like the stride: same trajectory, same arithmetic per substep.  Eight
+    segments, the last one ragged; a second backward on the same rollout (nothing on tape any more) must agree too."""
+    P = make_problem(cfg, batch=12, n_verts=40, horizon=H)
+    outs = []
+    for nbuf in ("1", "2", "3", "4"):
+        monkeypatch.setenv("DLO_TAPE_BUFFERS", nbuf)
+        sim = dlo.DloSim(P)
+        x = sim.rollout(H, stride).state()["x"]
+        _, seed = loss_and_seed(P, x)
+        outs.append(sim.backward(seed))
+        if nbuf == "4":
+            outs.append(sim.backward(seed))
+        assert sim.n_bad() == 0
+        sim.close()
+    assert np.abs(outs[0]["g_x0"]).max() > 0
+    for o in outs[1:]:
+        for k in ("g_actions", "g_x0", "g_v0", "g_material"):
+            assert np.abs(o[k] - outs[0][k]).max() <= 5e-5 * np.abs(outs[0][k]).max(), k
+
+
 @pytest.mark.parametrize("cfg, H, stride, tol", [(4, 400, 40, 5e-5), (5, 300, 100, 1e-3)])
 def test_side_records_equal_recompute(dlo, monkeypatch, cfg, H, stride, tol):
     """A substep that applied a self-contact correction is reversed either from the side record the replay left, or,
