@@ -301,7 +301,7 @@ def main():
         line["forward"] = {"value": res_f["value"], "unit": UNIT, "ms_per_step": res_f["ms_per_step"], "gpu_launches": res_f["launches"],
                            "ms_per_pass": res_f["ms_per_pass"], "roofline": kernel_roofline("k_forward", res_f["kernels"][0])}
     if not args.no_cpu_baseline:
-        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H, stride=stride), main_mode, budget_s=20)
+        cb, _, _ = oracle_leg(make_problem(args.config, batch=256, horizon=H, stride=stride), main_mode, budget_s=40)   # one pass of ~10-20 s
         line["cpu_baseline"] = cb
     print(json.dumps(line))
 
