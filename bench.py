@@ -243,6 +243,8 @@ def main():
             r["traffic"] = int(units // n * problem["config"]["n_substeps"] * rec_bytes)
             r["traffic_source"] = "tape layout: (22 + N_C) rows x NS x 4 B per env-substep x the env-substeps of one launch; ncu's dram bytes: profiles/"
             r["hbm_gbs"] = r["traffic"] / (tot_ms / n * 1e-3) / 1e9
+            # replays of earlier segments run on a second stream under the adjoints of later ones: both kernels' event times span that overlap
+            r["note"] = "launch durations include the time shared with the other stream's kernel (replay under adjoint); stand-alone durations: profiles/r02_ncu_summary.md"
         return r
 
     sampler = ClockSampler(local_rank)
