@@ -273,7 +273,7 @@ __device__ __noinline__ int build_pair_list(const KParams& __restrict__ P, int l
 // bound on dfar.  Too many near pairs for sm.hot: no near list (nhot = -1), dfar covers every pair.
 struct CandOut { int ncand, nhot; float dmin, dfar; };   // dmin: exact minimum segment distance over ALL eligible pairs, capped at 2(r_a+r_b); dfar: over the far ones
 template <int VPL>
-__device__ __noinline__ CandOut filter_candidates(const KParams& __restrict__ P, int lane, float* smbase, int nsurv, bool overflow) {
+__device__ __noinline__ CandOut filter_candidates(const KParams& __restrict__ P, int lane, float* smbase, int nsurv, bool overflow, bool wide) {
   WarpSmem sm;
   sm.init(P, smbase, 33 * VPL);
   const int N = P.N, NP = sm.NP;
@@ -290,8 +290,12 @@ __device__ __noinline__ CandOut filter_candidates(const KParams& __restrict__ P,
       c = surv[p];
       const int a = c >> 8, b = c & 255, an = (a + 1 < N) ? a + 1 : 0, bn = (b + 1 < N) ? b + 1 : 0;
       const float d2 = pair_dist2(sm.ys, NP, vpos<VPL>(a), vpos<VPL>(an), vpos<VPL>(b), vpos<VPL>(bn));
-      hit = d2 < lim * lim;
       near = d2 < near2;
+      // Candidates: by definition every pair closer than 2 (r_a + r_b) at x^p.  Only a pair that penetrates contributes, and
+      // while the corrections stay below (dfar - r_sum) / 2 no pair beyond the near distance can: the candidate list is then
+      // the near pairs alone (a handful instead of every pair of edges two apart), `wide` brings the others in when a
+      // projection loop does move that far (substep: far_unsafe after a build)
+      hit = wide ? d2 < lim * lim : near;
       d2min = fminf(d2min, d2);
       if (!near) d2far = fminf(d2far, d2);
     }
@@ -592,7 +596,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
   // correction changes nothing, so the state is identical to building the whole list and sweeping it every time.
   R.ncand = 0; R.any_pen = 0; R.jac_mask = 0u; R.work = 0; R.side_slot = -1;
   bool side_tried = false;
-  bool built = false;
+  bool built = false, wide_built = false;
   float D1 = 0.0f;
   float dnear = 1.0e30f;   // exact minimum distance at x^p over the pairs of the candidate list in use
   if (P.self_contact) {
@@ -602,7 +606,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       if (tp.vvalid[k]) { const f3 d = XP(k) - cc.xref[k]; m2 = fmaxf(m2, dot(d, d)); }
     D1 = sqrt_(warp_max(m2));
   }
-  auto build_list = [&](bool vote) {
+  auto build_list = [&](bool vote, bool wide) {
     // is the pair list still a superset?  (no vertex further than list_margin from where it was built)
     // (a list that was truncated is rebuilt at every use: that is this env's own business, the vote is about movement only)
     const bool trunc = cc.nlist < 0;
@@ -671,7 +675,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     float* oldd = sm.vs + P.hot_cap;
     for (int p = tp.lane; p < nold; p += 32) { oldc[p] = sm.cand[p]; oldd[p] = sm.dp[p]; }
     __syncwarp();
-    const CandOut co = filter_candidates<VPL>(P, tp.lane, sm.base, nuse, overflow);
+    const CandOut co = filter_candidates<VPL>(P, tp.lane, sm.base, nuse, overflow, wide);
     R.work += fresh ? 24 : 8;
     R.ncand = co.ncand;
     cc.dref = co.dfar;
@@ -695,7 +699,7 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
     const bool want = P.self_contact && !(cc.dref - 2.0f * D1 >= need);
     const bool go = (P.vote_mode & 1) ? phase_vote(sm, want) : want;
     if (go && P.self_contact) {
-      build_list((P.vote_mode & 1) != 0);
+      build_list((P.vote_mode & 1) != 0, false);
       built = true;
       D1 = 0.0f;
     } else if (P.self_contact && cc.nhot > 0) {
@@ -795,10 +799,15 @@ __device__ __forceinline__ void substep(const KParams& P, const Topo<VPL>& tp, c
       const float Dm = sqrt_(warp_max(m2)), need = 2.0f * P.r + 1.0e-6f;
       bool far_unsafe = !(cc.dref - 2.0f * (D1 + Dm) >= need);
       if (far_unsafe && !built) {
-        build_list(false);
+        build_list(false, false);
         built = true;
         D1 = 0.0f;
         far_unsafe = !(cc.dref - 2.0f * Dm >= need);
+      }
+      if (far_unsafe && !wide_built) {   // corrections so large that pairs beyond the near distance could touch: every pair closer than 2 (r_a + r_b) at x^p becomes a candidate
+        build_list(false, true);
+        built = true; wide_built = true;
+        D1 = 0.0f;
       }
       sweep = far_unsafe || !(dnear - 2.0f * Dm >= need);
     }
